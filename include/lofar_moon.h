@@ -1,0 +1,158 @@
+/*
+ * lofar_moon.h -- C ABI of the B200-native hot path of the LOFAR lunar-pulse trigger
+ * pipeline (arXiv 1612.06592, "Realtime processing of LOFAR data for the detection of
+ * nano-second pulses from the Moon").
+ *
+ * The path (section 2, "Overview of the online data analysis processing
+ * steps"): station sub-band voltages -> tied-array beams with the ionospheric
+ * de-dispersion phase folded into the per-sub-band weight (re-formulation of
+ * BASELINE.json:north_star) -> inversion of the polyphase filter, i.e. inverse Fourier
+ * transform + synthesis FIR (the FIR is the matched synthesis H^T, reading A8
+ * in DESIGN.md) -> amplitude trigger.
+ *
+ * Conventions
+ *   S stations, 2 polarisations, B beams, D STEC trials, K selected sub-bands k0..k0+K-1 of
+ *   an M = 1024 point critically sampled filter bank with P = 16 taps per branch,
+ *   T time slices per call.  nseries = B*D; series index = b*D + d.
+ *   f_sb(k) = f_zone + k*clock/M.
+ *
+ * Pointers: unless a parameter name ends in _host, every data pointer is a DEVICE pointer
+ * owned by the caller; the library never frees or reallocates caller memory.  The plan owns
+ * its tables, the carried PPF history, scratch and the streaming staging buffers.
+ * `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Stage
+ * calls only enqueue work on `stream` and return without synchronising.
+ *
+ * Errors: every call returns a lofar_status; nothing aborts or throws across the boundary.
+ * There is no CPU fallback: without a CUDA device the calls return LOFAR_E_CUDA.
+ * Calls on one plan must be issued from one thread at a time and, because the inverse PPF
+ * carries history, in stream order.
+ */
+#ifndef LOFAR_MOON_H
+#define LOFAR_MOON_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(LOFAR_MOON_BUILD)
+#define LOFAR_API __attribute__((visibility("default")))
+#else
+#define LOFAR_API
+#endif
+
+typedef struct lofar_plan lofar_plan; /* opaque, owned by the library */
+
+typedef enum {
+    LOFAR_OK = 0,
+    LOFAR_E_INVALID = 1,  /* NULL pointer, non-positive size, unsupported parameter value      */
+    LOFAR_E_SHAPE = 2,    /* sub-band range outside 0..M/2-1, slices > capacity, ...           */
+    LOFAR_E_ALIGN = 3,    /* X base or row pitch not 16-byte aligned                           */
+    LOFAR_E_ALLOC = 4,    /* host or device allocation failed                                  */
+    LOFAR_E_CUDA = 5,     /* a CUDA runtime call failed (sticky error left for the caller)     */
+    LOFAR_E_OVERFLOW = 6, /* more candidates than max_candidates (reported by lofar_stream_sync) */
+    LOFAR_E_STATE = 7     /* call not legal in the plan's current state                        */
+} lofar_status;
+
+typedef enum { LOFAR_CI8 = 0, LOFAR_CI16 = 1 } lofar_dtype;
+
+/* One trigger candidate (24 bytes).  With D > 1 trials only the best trial of a
+ * (beam, sample) is reported (BASELINE.json:configs[3], reading A15). */
+typedef struct {
+    uint32_t series; /* b*D + d                                                    */
+    uint32_t trial;  /* d                                                          */
+    uint64_t sample; /* global 5 ns index = stream offset + q*1024 + r             */
+    float env;       /* envelope e[n] (= |xhat[n]| for env_window 1)               */
+    float sigma;     /* sigma of that series over this block                       */
+} lofar_candidate;
+
+/* ---- plan ---------------------------------------------------------------------------------
+ * BASELINE.json:north_star: "lofar_plan_create(stations, subbands, beams, taps, STEC)".
+ * Creates a plan with one trial (D = 1) at stec_tecu, sub-bands k0 = 0..subbands-1 until
+ * lofar_plan_set_band moves them, zero delays, the default Kaiser prototype
+ * (BASELINE.json:configs[0]: 16384-tap windowed sinc, cutoff 1/1024, beta = 9), int8 input,
+ * kappa = 6, env_window = 1, max_candidates = 65536.  taps must be 16 (LOFAR_E_INVALID
+ * otherwise).  Device tables are built lazily at the first compute call. */
+LOFAR_API lofar_status lofar_plan_create(lofar_plan **out, int stations, int subbands, int beams,
+                                         int taps, double stec_tecu);
+LOFAR_API void lofar_plan_destroy(lofar_plan *plan);
+
+/* Setters copy their arguments.  Any of them invalidates the device tables; set_band,
+ * set_trials and set_input also reset the carried history (as lofar_stream_reset). */
+/* first_subband = k0 >= 0, k0 + K <= 512; fft_size must be 1024. */
+LOFAR_API lofar_status lofar_plan_set_band(lofar_plan *plan, int first_subband, double f_zone_hz,
+                                           double clock_hz, int fft_size);
+/* tau_s_host[beams][stations]: arrival lag in seconds of station s for beam b relative to the
+ * phase centre (reading A3/A4); weight W[b,s,k] = exp(+2 pi i f_sb(k) tau[b,s]). */
+LOFAR_API lofar_status lofar_plan_set_delays(lofar_plan *plan, const double *tau_s_host);
+/* D = ntrials >= 1 STEC values in TECU; Dph[d,k] = exp(-2 pi i 1.343e9 STEC_d / f_sb(k)). */
+LOFAR_API lofar_status lofar_plan_set_trials(lofar_plan *plan, int ntrials,
+                                             const double *stec_tecu_host);
+/* h_host[16*1024] analysis prototype (sum = 1); NULL restores the default Kaiser design.
+ * The synthesis taps are g = 1024*h (matched synthesis). */
+LOFAR_API lofar_status lofar_plan_set_filter(lofar_plan *plan, const double *h_host);
+/* Input sample type and the largest `slices` any later call will pass. */
+LOFAR_API lofar_status lofar_plan_set_input(lofar_plan *plan, lofar_dtype dtype, int max_slices);
+/* Threshold kappa (candidate iff e/sigma > kappa, strict), envelope window W >= 1 samples
+ * (e[n] = sqrt(mean of xhat[n-W+1..n]^2), reading A13), candidate buffer capacity. */
+LOFAR_API lofar_status lofar_plan_set_trigger(lofar_plan *plan, double kappa, int env_window,
+                                              uint32_t max_candidates);
+/* Device bytes the plan holds or will hold (tables + history + scratch + staging). */
+LOFAR_API lofar_status lofar_plan_workspace_bytes(lofar_plan *plan, size_t *bytes);
+
+/* ---- stage calls (all pointers device) ------------------------------------------------------
+ * X: [S][2][K][slices][re,im] int8 or int16, little endian, time fastest; base and row pitch
+ * (slices*2*sizeof(sample)) must be multiples of 16 bytes (LOFAR_E_ALIGN otherwise).
+ * Z: [B*D][K][slices] float2.   series: [B*D][slices*1024] float, sample n = q*1024 + r. */
+
+/* a1 + a2:  Z[b*D+d][k][q] = Dph[d,k] * sum_s sum_p W[b,s,k] X[s,p,k,q]. */
+LOFAR_API lofar_status lofar_beamform_dedisperse(lofar_plan *plan, const void *X, int slices,
+                                                 void *Z, void *stream);
+/* a3 + a4: per series and slice an unnormalised 1024-point Hermitian inverse
+ * DFT of the K selected bins (all other bins zero), then
+ * xhat[q*1024+r] = 1024 * sum_{t<16} h[r+1024 t] * y[q-t][r].  Reads and then replaces the
+ * plan's carried 15-slice history (zeros after lofar_stream_reset). */
+LOFAR_API lofar_status lofar_inverse_ppf(lofar_plan *plan, const void *Z, int slices, float *series,
+                                         void *stream);
+/* a5: envelope, sigma[series] = RMS of the envelope over this block,
+ * candidates e > kappa*sigma (best trial per (beam, sample) when D > 1), sorted by
+ * (beam, sample).  *count receives the true number of candidates; at most max_candidates
+ * records are stored (an unspecified subset, still sorted, when count > max_candidates).
+ * Candidate sample indices are stream offset + n; the stream offset advances by
+ * slices*1024 per lofar_trigger / lofar_run_block call. */
+LOFAR_API lofar_status lofar_trigger(lofar_plan *plan, const float *series, int slices,
+                                     lofar_candidate *cand, uint32_t *count, float *sigma,
+                                     void *stream);
+/* The whole chain on one block: a1..a5 with the beam sums kept in plan scratch. */
+LOFAR_API lofar_status lofar_run_block(lofar_plan *plan, const void *X, int slices, float *series,
+                                       lofar_candidate *cand, uint32_t *count, float *sigma,
+                                       void *stream);
+
+/* ---- streaming driver (a6; BASELINE.json:configs[4]) -------------------------------------------
+ * lofar_stream_reset: waits for the plan's own streams, zeroes the carried history and the
+ * stream offset.
+ * lofar_stream_push: X_host is a HOST buffer (pinned for copy/compute overlap; pageable works
+ * but serialises) laid out as X above.  The block is copied into one of two plan-owned device
+ * buffers on a copy stream while the previous block computes on a compute stream; then
+ * lofar_run_block runs on it; then count, sigma[B*D] and the stored candidates are copied to
+ * the *_host buffers (any of which may be NULL).  series is a device buffer (never copied to
+ * the host).  Returns without waiting.  Host result buffers and X_host must stay untouched
+ * until lofar_stream_sync returns.
+ * lofar_stream_sync: blocks until all pushed blocks are done; returns LOFAR_E_OVERFLOW if any
+ * block since the last sync had more candidates than max_candidates. */
+LOFAR_API lofar_status lofar_stream_reset(lofar_plan *plan);
+LOFAR_API lofar_status lofar_stream_push(lofar_plan *plan, const void *X_host, int slices,
+                                         float *series, lofar_candidate *cand_host,
+                                         uint32_t *count_host, float *sigma_host);
+LOFAR_API lofar_status lofar_stream_sync(lofar_plan *plan);
+
+/* Number of kernel launches the plan has enqueued so far (for bench accounting). */
+LOFAR_API uint64_t lofar_plan_launch_count(const lofar_plan *plan);
+LOFAR_API const char *lofar_status_string(lofar_status status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LOFAR_MOON_H */

@@ -1,0 +1,232 @@
+"""Thin ctypes binding of the C-ABI library (include/lofar_moon.h).  Argument marshalling only:
+every step of the path runs in the CUDA kernels behind the boundary.  Same names as the C calls.
+
+torch is used for device memory and streams (tensors in, tensors out); nothing here computes.
+`load()` fails loudly if liblofar_moon.so is missing -- there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblofar_moon.so")
+
+LOFAR_OK, LOFAR_E_INVALID, LOFAR_E_SHAPE, LOFAR_E_ALIGN, LOFAR_E_ALLOC, LOFAR_E_CUDA, \
+    LOFAR_E_OVERFLOW, LOFAR_E_STATE = range(8)
+LOFAR_CI8, LOFAR_CI16 = 0, 1
+
+# numpy view of lofar_candidate (24 bytes)
+CANDIDATE_DTYPE = np.dtype([("series", "<u4"), ("trial", "<u4"), ("sample", "<u8"),
+                            ("env", "<f4"), ("sigma", "<f4")])
+assert CANDIDATE_DTYPE.itemsize == 24
+
+EXPORTS = (
+    "lofar_plan_create", "lofar_plan_destroy", "lofar_plan_set_band", "lofar_plan_set_delays",
+    "lofar_plan_set_trials", "lofar_plan_set_filter", "lofar_plan_set_input",
+    "lofar_plan_set_trigger", "lofar_plan_workspace_bytes", "lofar_beamform_dedisperse",
+    "lofar_inverse_ppf", "lofar_trigger", "lofar_run_block", "lofar_stream_reset",
+    "lofar_stream_push", "lofar_stream_sync", "lofar_plan_launch_count", "lofar_status_string",
+)
+
+
+class LofarError(RuntimeError):
+    def __init__(self, status: int, call: str):
+        self.status = status
+        super().__init__(f"{call}: {status_string(status)} (status {status})")
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """Load liblofar_moon.so (build it with `python -m paper_1612_06592_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1612_06592_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    c = ctypes
+    vp, i, d, u32, u64 = c.c_void_p, c.c_int, c.c_double, c.c_uint32, c.c_uint64
+    sig = {
+        "lofar_plan_create": (i, [c.POINTER(vp), i, i, i, i, d]),
+        "lofar_plan_destroy": (None, [vp]),
+        "lofar_plan_set_band": (i, [vp, i, d, d, i]),
+        "lofar_plan_set_delays": (i, [vp, vp]),
+        "lofar_plan_set_trials": (i, [vp, i, vp]),
+        "lofar_plan_set_filter": (i, [vp, vp]),
+        "lofar_plan_set_input": (i, [vp, i, i]),
+        "lofar_plan_set_trigger": (i, [vp, d, i, u32]),
+        "lofar_plan_workspace_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
+        "lofar_beamform_dedisperse": (i, [vp, vp, i, vp, vp]),
+        "lofar_inverse_ppf": (i, [vp, vp, i, vp, vp]),
+        "lofar_trigger": (i, [vp, vp, i, vp, vp, vp, vp]),
+        "lofar_run_block": (i, [vp, vp, i, vp, vp, vp, vp, vp]),
+        "lofar_stream_reset": (i, [vp]),
+        "lofar_stream_push": (i, [vp, vp, i, vp, vp, vp, vp]),
+        "lofar_stream_sync": (i, [vp]),
+        "lofar_plan_launch_count": (u64, [vp]),
+        "lofar_status_string": (c.c_char_p, [i]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(lib, name)
+        f.restype = res
+        f.argtypes = args
+    _lib = lib
+    return lib
+
+
+def status_string(status: int) -> str:
+    return load().lofar_status_string(int(status)).decode()
+
+
+def _check(status: int, call: str, allow=()):
+    if status != LOFAR_OK and status not in allow:
+        raise LofarError(status, call)
+    return status
+
+
+def _ptr(t) -> int:
+    """Device (or pinned host) address of a torch tensor / numpy array; None -> NULL."""
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data
+    assert t.is_contiguous()
+    return t.data_ptr()
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream or None
+
+
+class Plan:
+    """Owns one lofar_plan*.  Methods carry the names of the C calls they forward to."""
+
+    def __init__(self, stations: int, subbands: int, beams: int, taps: int = 16, stec_tecu: float = 0.0):
+        self._lib = load()
+        h = ctypes.c_void_p()
+        _check(self._lib.lofar_plan_create(ctypes.byref(h), stations, subbands, beams, taps, float(stec_tecu)),
+               "lofar_plan_create")
+        self._h = h
+        self.S, self.K, self.B, self.D = stations, subbands, beams, 1
+        self.max_candidates = 65536
+
+    # -- lifetime
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.lofar_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    @property
+    def nseries(self) -> int:
+        return self.B * self.D
+
+    # -- setters
+    def set_band(self, first_subband: int, f_zone_hz: float = 100e6, clock_hz: float = 200e6, fft_size: int = 1024):
+        _check(self._lib.lofar_plan_set_band(self._h, first_subband, f_zone_hz, clock_hz, fft_size), "lofar_plan_set_band")
+
+    def set_delays(self, tau_s):
+        tau = np.ascontiguousarray(tau_s, dtype=np.float64)
+        assert tau.shape == (self.B, self.S)
+        _check(self._lib.lofar_plan_set_delays(self._h, tau.ctypes.data), "lofar_plan_set_delays")
+
+    def set_trials(self, stec_tecu):
+        st = np.ascontiguousarray(np.atleast_1d(stec_tecu), dtype=np.float64)
+        _check(self._lib.lofar_plan_set_trials(self._h, st.size, st.ctypes.data), "lofar_plan_set_trials")
+        self.D = int(st.size)
+
+    def set_filter(self, h=None):
+        if h is None:
+            _check(self._lib.lofar_plan_set_filter(self._h, None), "lofar_plan_set_filter")
+        else:
+            hh = np.ascontiguousarray(h, dtype=np.float64)
+            assert hh.size == 16 * 1024
+            _check(self._lib.lofar_plan_set_filter(self._h, hh.ctypes.data), "lofar_plan_set_filter")
+
+    def set_input(self, dtype: int, max_slices: int):
+        _check(self._lib.lofar_plan_set_input(self._h, dtype, max_slices), "lofar_plan_set_input")
+
+    def set_trigger(self, kappa: float, env_window: int = 1, max_candidates: int = 65536):
+        _check(self._lib.lofar_plan_set_trigger(self._h, float(kappa), env_window, max_candidates), "lofar_plan_set_trigger")
+        self.max_candidates = max_candidates
+
+    def workspace_bytes(self) -> int:
+        n = ctypes.c_size_t()
+        _check(self._lib.lofar_plan_workspace_bytes(self._h, ctypes.byref(n)), "lofar_plan_workspace_bytes")
+        return int(n.value)
+
+    def launch_count(self) -> int:
+        return int(self._lib.lofar_plan_launch_count(self._h))
+
+    # -- stage calls (device tensors; raw status codes via `allow` for error-path tests)
+    def beamform_dedisperse(self, X, slices: int, Z, stream=None, allow=()):
+        return _check(self._lib.lofar_beamform_dedisperse(self._h, _ptr(X), slices, _ptr(Z), _stream_ptr(stream)),
+                      "lofar_beamform_dedisperse", allow)
+
+    def inverse_ppf(self, Z, slices: int, series, stream=None, allow=()):
+        return _check(self._lib.lofar_inverse_ppf(self._h, _ptr(Z), slices, _ptr(series), _stream_ptr(stream)),
+                      "lofar_inverse_ppf", allow)
+
+    def trigger(self, series, slices: int, cand, count, sigma, stream=None, allow=()):
+        return _check(self._lib.lofar_trigger(self._h, _ptr(series), slices, _ptr(cand), _ptr(count), _ptr(sigma),
+                                              _stream_ptr(stream)), "lofar_trigger", allow)
+
+    def run_block(self, X, slices: int, series, cand, count, sigma, stream=None, allow=()):
+        return _check(self._lib.lofar_run_block(self._h, _ptr(X), slices, _ptr(series), _ptr(cand), _ptr(count),
+                                                _ptr(sigma), _stream_ptr(stream)), "lofar_run_block", allow)
+
+    # -- streaming
+    def stream_reset(self):
+        _check(self._lib.lofar_stream_reset(self._h), "lofar_stream_reset")
+
+    def stream_push(self, X_host, slices: int, series, cand_host=None, count_host=None, sigma_host=None, allow=()):
+        return _check(self._lib.lofar_stream_push(self._h, _ptr(X_host), slices, _ptr(series), _ptr(cand_host),
+                                                  _ptr(count_host), _ptr(sigma_host)), "lofar_stream_push", allow)
+
+    def stream_sync(self, allow=()):
+        return _check(self._lib.lofar_stream_sync(self._h), "lofar_stream_sync", allow)
+
+
+def plan_for(w, tau) -> Plan:
+    """Plan configured for a synth.Workload (marshalling of its parameters, nothing else)."""
+    p = Plan(w.S, w.K, w.B, w.P, w.stec[0])
+    p.set_band(w.k0)
+    p.set_delays(tau)
+    if w.D > 1:
+        p.set_trials(np.asarray(w.stec, dtype=np.float64))
+    p.set_input(LOFAR_CI16 if w.dtype == "ci16" else LOFAR_CI8, w.T)
+    p.set_trigger(w.kappa, 1, 65536)
+    return p
+
+
+def new_outputs(plan: Plan, slices: int, device="cuda"):
+    """Allocate the caller-owned output buffers of run_block as torch tensors."""
+    import torch
+    series = torch.empty((plan.nseries, slices * 1024), dtype=torch.float32, device=device)
+    cand = torch.zeros((plan.max_candidates, 24), dtype=torch.uint8, device=device)
+    count = torch.zeros(1, dtype=torch.int32, device=device)
+    sigma = torch.zeros(plan.nseries, dtype=torch.float32, device=device)
+    return series, cand, count, sigma
+
+
+def candidates_to_numpy(cand, count) -> np.ndarray:
+    """Copy the stored candidate records to a structured numpy array (device -> host copy only)."""
+    n = int(count.item()) if hasattr(count, "item") else int(count)
+    raw = cand.cpu().numpy() if hasattr(cand, "cpu") else np.asarray(cand)
+    rec = raw.reshape(-1).view(CANDIDATE_DTYPE)
+    return rec[:min(n, rec.size)].copy()

@@ -1,0 +1,116 @@
+// plan.h -- internal plan object and the launcher prototypes of the kernel translation units.
+// Not part of the public boundary (include/lofar_moon.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <vector>
+
+#include "../../include/lofar_moon.h"
+
+namespace lofar {
+
+// ---- launch parameter blocks -------------------------------------------------------------------
+struct BeamformArgs {
+    const void *X;        // [S][2][K][xpitch] complex ints
+    long long xpitch;     // samples per input row
+    long long t0;         // first slice of this launch inside X rows
+    long long nt;         // slices to process
+    float2 *Z;            // [nz][K][zpitch], slice t0+i stored at column i
+    long long zpitch;
+    const float2 *W;      // [K][B][S] weights (de-dispersion phase folded in when D == 1)
+    const float2 *Dph;    // [D][K] trial phasors, used when nphase > 0
+    int S, K, B;
+    int nphase;           // 0: write the B beam sums; D > 0: write B*D phased series (stage call, D > 1)
+    int dtype;            // LOFAR_CI8 / LOFAR_CI16
+};
+
+struct IppfArgs {
+    const float2 *Z;      // [nz][K][zpitch]
+    long long zpitch;
+    long long nc;         // slices in this launch (columns 0..nc-1 of Z)
+    float *series;        // [nseries][series_pitch]; this launch writes samples out0 .. out0 + nc*1024
+    long long series_pitch;
+    long long out0;
+    const float2 *Dph;    // [D][K]; applied on load when zmap_trials != 0
+    int zmap_trials;      // 0: Z holds one row set per series;  D: Z holds per-beam sums, series = b*D+d
+    int K, k0, nseries;
+    int nspans, span_len; // span_len is a multiple of 16
+    const float *hist_in; // [nseries][15][1024]
+    float *hist_out;
+    const float2 *gs;     // [16][512] synthesis taps (g[2n + 1024 t], g[2n+1 + 1024 t])
+    const float2 *tw;     // twiddles: w1024[256], T2[7][8], T3[7][64]
+    double *partial;      // [nseries][partial_pitch] sum of xhat^2 per CTA
+    int partial_pitch, partial0;
+    float *chunkmax;      // [nseries][chunkmax_pitch] max |xhat| per 16-slice step
+    long long chunkmax_pitch, step0;
+    int vec_ok;           // Z rows allow 16-byte loads
+};
+
+struct TriggerArgs {
+    const float *series;  // [nseries][series_pitch]
+    long long series_pitch;
+    long long N;          // samples per series in this block
+    int B, D, W;          // beams, trials, envelope window
+    float kappa;
+    const float *tail;    // [nseries][W-1] samples preceding the block (W > 1)
+    double *partial;      // [nseries][partial_pitch]
+    int partial_pitch, nparts;
+    float *chunkmax;      // [nseries][chunkmax_pitch], one per 16384 samples
+    long long chunkmax_pitch, nchunks;
+    float *sigma;         // [nseries]
+    lofar_candidate *cand;
+    uint32_t *count;
+    uint32_t cap;
+    uint64_t offset;      // stream offset of sample 0 of this block
+};
+
+// kernel launchers (each returns the number of kernels it launched, or -1 on a launch error)
+int launch_beamform(const BeamformArgs &a, cudaStream_t st);
+int launch_ippf(const IppfArgs &a, cudaStream_t st);
+int ippf_configure();                                   // opt in to the large dynamic shared memory
+int launch_trigger_reduce(const TriggerArgs &a, cudaStream_t st);   // sum e^2 + chunk max from the series
+int launch_trigger_finish(const TriggerArgs &a, cudaStream_t st);   // sigma, threshold scan, sort
+int launch_tail_save(const float *series, long long pitch, long long N, int nseries, int W,
+                     float *tail, cudaStream_t st);
+
+}  // namespace lofar
+
+struct lofar_plan {
+    // problem
+    int S = 0, K = 0, B = 0, D = 1, P = 16, M = 1024, k0 = 0;
+    double f_zone = 100e6, clock = 200e6;
+    std::vector<double> tau, stec, h;
+    lofar_dtype dtype = LOFAR_CI8;
+    int max_slices = 0;
+    double kappa = 6.0;
+    int env_window = 1;
+    uint32_t max_cand = 65536;
+    // device state
+    bool built = false;
+    int num_sms = 148;
+    float2 *dW = nullptr, *dDph = nullptr, *dGs = nullptr, *dTw = nullptr;
+    float *dHist[2] = {nullptr, nullptr};
+    int hist_parity = 0;
+    float *dTail = nullptr;
+    float2 *dZ = nullptr;
+    long long zchunk = 0;          // slices per scratch chunk
+    double *dPartial = nullptr;
+    int partial_pitch = 0;
+    float *dChunkMax = nullptr;
+    long long chunkmax_pitch = 0;
+    size_t device_bytes = 0;
+    uint64_t offset = 0;
+    uint64_t launches = 0;
+    // streaming
+    cudaStream_t s_copy = nullptr, s_comp = nullptr;
+    void *dX[2] = {nullptr, nullptr};
+    size_t dX_bytes = 0;
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+    bool slot_used[2] = {false, false};
+    lofar_candidate *dCand[2] = {nullptr, nullptr};
+    uint32_t *dCount[2] = {nullptr, nullptr};
+    float *dSigma[2] = {nullptr, nullptr};
+    uint32_t *hCount = nullptr;    // pinned, one per push since the last sync (ring of 64)
+    int pushes = 0;
+    uint64_t push_index = 0;
+};

@@ -324,3 +324,26 @@ def generate_timedomain(w: Workload, tau: np.ndarray | None = None) -> np.ndarra
             v = np.stack([Y.real, Y.imag], axis=-1)
             X[s, p] = np.clip(np.rint(v), -w.clip, w.clip)
     return X
+
+
+# ----------------------------------------------------------------------------- stage-level inputs
+def random_z(seed: int, nseries: int, K: int, T: int, scale: float = 30.0) -> np.ndarray:
+    """Seeded complex64 beam sums Z[nseries][K][T] for testing the inverse PPF on its own
+    (white, the level of 48 summed int8 streams)."""
+    rng = np.random.default_rng(BASE_SEED + 7000 + seed)
+    z = rng.standard_normal((nseries, K, T, 2), dtype=np.float32) * np.float32(scale)
+    return z.view(np.complex64).reshape(nseries, K, T)
+
+
+def random_series(seed: int, nseries: int, N: int, spikes: int = 6, level: float = 9.0) -> np.ndarray:
+    """Seeded float32 series[nseries][N]: unit white noise plus a few spikes of +-level (some placed
+    at the same sample in several series, some near the block edges) for testing the trigger alone."""
+    rng = np.random.default_rng(BASE_SEED + 8000 + seed)
+    x = rng.standard_normal((nseries, N), dtype=np.float32)
+    for i in range(spikes):
+        n = int(rng.integers(0, N)) if i >= 2 else (0 if i == 0 else N - 1)
+        amp = level * (1.0 + 0.2 * rng.random())
+        for s in range(nseries):
+            if i % 2 == 0 or s == int(rng.integers(0, nseries)):
+                x[s, n] = np.float32(amp * (1 if rng.random() < 0.5 else -1) * (1.0 + 0.05 * s))
+    return x
