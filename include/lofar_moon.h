@@ -79,8 +79,8 @@ LOFAR_API lofar_status lofar_plan_create(lofar_plan **out, int stations, int sub
                                          int taps, double stec_tecu);
 LOFAR_API void lofar_plan_destroy(lofar_plan *plan);
 
-/* Setters copy their arguments.  Any of them invalidates the device tables; set_band,
- * set_trials and set_input also reset the carried history (as lofar_stream_reset). */
+/* Setters copy their arguments.  Any of them invalidates the device tables;
+ * every setter also resets the carried history and the stream offset (as lofar_stream_reset). */
 /* first_subband = k0 >= 0, k0 + K <= 512; fft_size must be 1024. */
 LOFAR_API lofar_status lofar_plan_set_band(lofar_plan *plan, int first_subband, double f_zone_hz,
                                            double clock_hz, int fft_size);
@@ -148,6 +148,12 @@ LOFAR_API lofar_status lofar_stream_push(lofar_plan *plan, const void *X_host, i
                                          uint32_t *count_host, float *sigma_host);
 LOFAR_API lofar_status lofar_stream_sync(lofar_plan *plan);
 
+/* Per-kernel device timing (measurement aid, PAPER-independent).  With profiling enabled every kernel
+ * the plan launches is bracketed by CUDA events on its own stream.  lofar_plan_profile_read waits for
+ * the recorded events, ADDS the elapsed milliseconds and launch counts since the previous read to
+ * ms_host[3] / launches_host[3] (index 0 beamform, 1 inverse PPF, 2 trigger kernels) and clears them. */
+LOFAR_API lofar_status lofar_plan_profile(lofar_plan *plan, int enable);
+LOFAR_API lofar_status lofar_plan_profile_read(lofar_plan *plan, double *ms_host, uint64_t *launches_host);
 /* Number of kernel launches the plan has enqueued so far (for bench accounting). */
 LOFAR_API uint64_t lofar_plan_launch_count(const lofar_plan *plan);
 LOFAR_API const char *lofar_status_string(lofar_status status);

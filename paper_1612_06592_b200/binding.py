@@ -28,7 +28,8 @@ EXPORTS = (
     "lofar_plan_set_trials", "lofar_plan_set_filter", "lofar_plan_set_input",
     "lofar_plan_set_trigger", "lofar_plan_workspace_bytes", "lofar_beamform_dedisperse",
     "lofar_inverse_ppf", "lofar_trigger", "lofar_run_block", "lofar_stream_reset",
-    "lofar_stream_push", "lofar_stream_sync", "lofar_plan_launch_count", "lofar_status_string",
+    "lofar_stream_push", "lofar_stream_sync", "lofar_plan_profile", "lofar_plan_profile_read",
+    "lofar_plan_launch_count", "lofar_status_string",
 )
 
 
@@ -69,6 +70,8 @@ def load() -> ctypes.CDLL:
         "lofar_stream_reset": (i, [vp]),
         "lofar_stream_push": (i, [vp, vp, i, vp, vp, vp, vp]),
         "lofar_stream_sync": (i, [vp]),
+        "lofar_plan_profile": (i, [vp, i]),
+        "lofar_plan_profile_read": (i, [vp, vp, vp]),
         "lofar_plan_launch_count": (u64, [vp]),
         "lofar_status_string": (c.c_char_p, [i]),
     }
@@ -172,6 +175,16 @@ class Plan:
 
     def launch_count(self) -> int:
         return int(self._lib.lofar_plan_launch_count(self._h))
+
+    def profile(self, enable: bool):
+        _check(self._lib.lofar_plan_profile(self._h, int(enable)), "lofar_plan_profile")
+
+    def profile_read(self):
+        """(ms[3], launches[3]) accumulated since the previous read: beamform, inverse PPF, trigger."""
+        ms = np.zeros(3, dtype=np.float64)
+        n = np.zeros(3, dtype=np.uint64)
+        _check(self._lib.lofar_plan_profile_read(self._h, ms.ctypes.data, n.ctypes.data), "lofar_plan_profile_read")
+        return ms, n
 
     # -- stage calls (device tensors; raw status codes via `allow` for error-path tests)
     def beamform_dedisperse(self, X, slices: int, Z, stream=None, allow=()):

@@ -80,6 +80,26 @@ float2 unit_phasor(double turns)
     return make_float2((float)std::cos(kTwoPi * turns), (float)std::sin(kTwoPi * turns));
 }
 
+// Brackets the kernels launched inside its lifetime with two events on their stream.
+struct ProfScope {
+    lofar_plan *p; int id; cudaStream_t st; cudaEvent_t a = nullptr, b = nullptr;
+    static cudaEvent_t take(lofar_plan *p)
+    {
+        cudaEvent_t e = nullptr;
+        if (!p->prof_pool.empty()) { e = p->prof_pool.back(); p->prof_pool.pop_back(); }
+        else cudaEventCreate(&e);
+        return e;
+    }
+    ProfScope(lofar_plan *p_, int id_, cudaStream_t st_) : p(p_), id(id_), st(st_)
+    {
+        if (p->prof) { a = take(p); b = take(p); cudaEventRecord(a, st); }
+    }
+    ~ProfScope()
+    {
+        if (a) { cudaEventRecord(b, st); p->prof_pending.push_back({id, a, b}); }
+    }
+};
+
 long long round_up(long long v, long long m) { return (v + m - 1) / m * m; }
 
 size_t sample_bytes(const lofar_plan *p) { return p->dtype == LOFAR_CI16 ? 4 : 2; }
@@ -195,6 +215,7 @@ lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, long long
     a.partial = p->dPartial; a.partial_pitch = p->partial_pitch; a.partial0 = *partial0;
     a.chunkmax = p->dChunkMax; a.chunkmax_pitch = p->chunkmax_pitch; a.step0 = step0;
     a.vec_ok = ((zpitch & 1) == 0) && ((reinterpret_cast<size_t>(Z) & 15) == 0);
+    ProfScope prof(p, 1, st);
     const int n = launch_ippf(a, st);
     if (n < 0) return LOFAR_E_CUDA;
     p->launches += n;
@@ -238,15 +259,19 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
         b.Z = p->dZ; b.zpitch = p->zchunk;
         b.W = p->dW; b.Dph = p->dDph;
         b.S = p->S; b.K = p->K; b.B = p->B; b.nphase = 0; b.dtype = p->dtype;
-        const int n = launch_beamform(b, st);
-        if (n < 0) return LOFAR_E_CUDA;
-        p->launches += n;
+        {
+            ProfScope prof(p, 0, st);
+            const int n = launch_beamform(b, st);
+            if (n < 0) return LOFAR_E_CUDA;
+            p->launches += n;
+        }
         lofar_status s = do_ippf(p, p->dZ, p->zchunk, nc, p->D > 1 ? p->D : 0, series, N, c0 * kMfft, &partial0,
                                  c0 / kStepSlices, st);
         if (s != LOFAR_OK) return s;
     }
     TriggerArgs t = trigger_args(p, series, N, cand, count, sigma);
     int n;
+    ProfScope prof(p, 2, st);
     if (p->env_window == 1) {
         t.nparts = partial0;
     } else {
@@ -297,6 +322,8 @@ void lofar_plan_destroy(lofar_plan *p)
         if (p->ev_done[i]) cudaEventDestroy(p->ev_done[i]);
     }
     if (p->hCount) cudaFreeHost(p->hCount);
+    for (auto &r : p->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto e : p->prof_pool) cudaEventDestroy(e);
     free_tables(p);
     delete p;
 }
@@ -386,6 +413,7 @@ lofar_status lofar_beamform_dedisperse(lofar_plan *p, const void *X, int slices,
     b.Z = static_cast<float2 *>(Z); b.zpitch = slices;
     b.W = p->dW; b.Dph = p->dDph;
     b.S = p->S; b.K = p->K; b.B = p->B; b.nphase = p->D > 1 ? p->D : 0; b.dtype = p->dtype;
+    ProfScope prof(p, 0, static_cast<cudaStream_t>(stream));
     const int n = launch_beamform(b, static_cast<cudaStream_t>(stream));
     if (n < 0) return LOFAR_E_CUDA;
     p->launches += n;
@@ -414,6 +442,7 @@ lofar_status lofar_trigger(lofar_plan *p, const float *series, int slices, lofar
     TriggerArgs t = trigger_args(p, series, N, cand, count, sigma);
     t.nparts = (int)t.nchunks;
     int n;
+    ProfScope prof(p, 2, st);
     if ((n = launch_trigger_reduce(t, st)) < 0) return LOFAR_E_CUDA;
     p->launches += n;
     if ((n = launch_trigger_finish(t, st)) < 0) return LOFAR_E_CUDA;
@@ -517,6 +546,28 @@ lofar_status lofar_stream_sync(lofar_plan *p)
     for (int i = 0; i < p->pushes; ++i) over = over || (p->hCount[i] > p->max_cand);
     p->pushes = 0;
     return over ? LOFAR_E_OVERFLOW : LOFAR_OK;
+}
+
+lofar_status lofar_plan_profile(lofar_plan *p, int enable)
+{
+    if (!p) return LOFAR_E_INVALID;
+    p->prof = enable != 0;
+    return LOFAR_OK;
+}
+
+lofar_status lofar_plan_profile_read(lofar_plan *p, double *ms, uint64_t *launches)
+{
+    if (!p || !ms || !launches) return LOFAR_E_INVALID;
+    for (auto &r : p->prof_pending) {
+        float t = 0.f;
+        CU(cudaEventSynchronize(r.b));
+        CU(cudaEventElapsedTime(&t, r.a, r.b));
+        if (r.id >= 0 && r.id < 3) { ms[r.id] += (double)t; launches[r.id] += 1; }
+        p->prof_pool.push_back(r.a);
+        p->prof_pool.push_back(r.b);
+    }
+    p->prof_pending.clear();
+    return LOFAR_OK;
 }
 
 uint64_t lofar_plan_launch_count(const lofar_plan *p) { return p ? p->launches : 0; }

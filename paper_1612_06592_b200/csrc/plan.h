@@ -113,4 +113,9 @@ struct lofar_plan {
     uint32_t *hCount = nullptr;    // pinned, one per push since the last sync (ring of 64)
     int pushes = 0;
     uint64_t push_index = 0;
+    // per-kernel profiling (lofar_plan_profile)
+    bool prof = false;
+    struct ProfRec { int id; cudaEvent_t a, b; };
+    std::vector<ProfRec> prof_pending;
+    std::vector<cudaEvent_t> prof_pool;
 };

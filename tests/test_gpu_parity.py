@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 
 from paper_1612_06592_b200 import binding, synth
-from tests.parity_util import assert_close, check_candidates, oracle_snr
+from parity_util import assert_close, check_candidates, oracle_snr
 
 pytestmark = pytest.mark.gpu
 
@@ -98,7 +98,7 @@ def test_inverse_ppf_parity_and_history(torch, oracle, kw):
 def test_trigger_parity(torch, oracle, D, Wn, N):
     B = 3
     ns = B * D
-    kappa = 5.0
+    kappa = 5.0 if Wn == 1 else 2.5      # a one-sample spike of 9 sigma is 9/sqrt(W) in the envelope
     p = binding.Plan(2, 8, B, 16, 5.0)
     if D > 1:
         p.set_trials(np.arange(5.0, 5.0 + D))
