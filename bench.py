@@ -1,0 +1,317 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path (beamform+de-dispersion -> inverse PPF -> trigger) on
+synthetic LOFAR-shaped data, per the driver contract.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl reference]
+
+A step is one lofar_run_block over one block of the workload (default: BASELINE.json:configs[2], the
+24 stations x 488 sub-bands x 24 beams case the north_star target names).  `value` is reconstructed
+5 ns samples/s per beam with the input resident in HBM; `e2e` is the same through lofar_stream_push
+with the block in pinned HOST memory (H2D inside the timed region, candidates/sigma copied back).
+N > 1: the path has no sharding or collectives (north_star) -> N independent replicas, one per GPU.
+`--impl reference` times the CPU oracle on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1612_06592_b200 import synth  # noqa: E402
+
+METRIC = "reconstructed 5 ns samples/s per beam"
+UNIT = "samples/s/beam"
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def workload(idx: int, slices: int | None):
+    w = synth.config(idx)
+    if slices:
+        from dataclasses import replace
+        w = replace(w, T=slices)
+    return w
+
+
+def describe(w, extra=None):
+    d = {"workload": f"configs[{w.index}] {w.name}: S={w.S} pols=2 B={w.B} D={w.D} K={w.K} (k0={w.k0}) "
+                     f"T={w.T} slices/block {w.dtype}",
+         "stations": w.S, "beams": w.B, "trials": w.D, "subbands": w.K, "slices_per_block": w.T,
+         "input_dtype": w.dtype, "block_seconds_of_data": w.T * w.slice_seconds,
+         "l2": "inputs larger than L2 (no flush needed)" if w.input_bytes > 256e6 else "flushed"}
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        self.p.wait()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[2:6]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------- oracle legs
+def oracle_sample(w, X_sample, tau, budget_s=15.0):
+    """Times the oracle as it stands on a bounded sample (the first `nq` slices of the block, all
+    stations/sub-bands/beams/trials); returns (samples/s/beam, cores, description, seconds)."""
+    from oracle import lofar_oracle as oracle
+    pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa)
+    nq = 4
+    t0 = time.perf_counter()
+    pipe.run_block(np.ascontiguousarray(X_sample[:, :, :, :nq]))
+    probe = time.perf_counter() - t0
+    per_slice = max(probe / nq, 1e-6)
+    nq = int(min(X_sample.shape[3], max(8, budget_s / per_slice)))
+    pipe.reset()
+    xs = np.ascontiguousarray(X_sample[:, :, :, :nq])
+    t0 = time.perf_counter()
+    pipe.run_block(xs)
+    dt = time.perf_counter() - t0
+    return nq * w.M / dt, oracle.threads(), f"first {nq} slices of one block, all {w.nseries} series", dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = workload(args.config, args.slices)
+    _, _, tau = synth.geometry(w)
+    from dataclasses import replace
+    ws = replace(w, T=min(w.T, 2048))
+    X = synth.generate_block(ws, 0, tau=tau)
+    vals, cores, sample = [], 1, ""
+    budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for i in range(args.warmup + args.steps):
+        v, cores, sample, dt = oracle_sample(w, X, tau, budget)
+        if i >= args.warmup:
+            vals.append((v, dt))
+    value = float(np.mean([v for v, _ in vals]))
+    ms = float(np.mean([dt for _, dt in vals]) * 1e3)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, paper_1612_06592_b200.synth)",
+        "config": describe(w, {"note": "each step is a bounded sample of the block"}),
+        "real_time_factor": value / 200e6,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ------------------------------------------------------------------------------------- GPU arm
+def run_gpu(args):
+    import torch
+    from paper_1612_06592_b200 import binding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+    binding.load()
+
+    w = workload(args.config, args.slices)
+    _, _, tau = synth.geometry(w)
+    X = synth.generate_block(w, 0, tau=tau)
+    plan = binding.plan_for(w, tau)
+    cap = 4096
+    plan.set_trigger(w.kappa, 1, cap)
+    Xd = torch.from_numpy(X).cuda()
+    series, cand, count, sigma = binding.new_outputs(plan, w.T)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        plan.run_block(Xd, w.T, series, cand, count, sigma, stream)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    plan.profile(True)
+    plan.profile_read()
+    l0 = plan.launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    launches = plan.launch_count() - l0
+    kms, kn = plan.profile_read()
+    plan.profile(False)
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    n_cand = int(count.item())
+
+    # ---- e2e: the same step through lofar_stream_push from pinned host memory
+    Xh = torch.from_numpy(X).pin_memory()
+    cand_h = torch.zeros((cap, 24), dtype=torch.uint8).pin_memory()
+    count_h = torch.zeros(1, dtype=torch.int32).pin_memory()
+    sigma_h = torch.zeros(w.nseries, dtype=torch.float32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 5))
+    plan.stream_reset()
+    for _ in range(2):
+        plan.stream_push(Xh, w.T, series, cand_h, count_h, sigma_h)
+    plan.stream_sync()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        plan.stream_push(Xh, w.T, series, cand_h, count_h, sigma_h)
+    plan.stream_sync()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_ms = e2e_s / e2e_steps * 1e3
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    samples_per_block = w.T * w.M
+    value = world * samples_per_block / (ms_step * 1e-3)            # per beam, all replicas
+    e2e_value = world * samples_per_block / (e2e_ms * 1e-3)
+    peak, peak_src = peaks()
+
+    # algorithmic bytes per launch
+    esz = 4 if w.dtype == "ci16" else 2
+    zrows = w.B                                   # beam sums are written once per beam, trials fan out on load
+    by_kernel = {
+        "beamform_kernel": w.S * 2 * w.K * w.T * esz + zrows * w.K * w.T * 8,
+        "ippf_kernel": zrows * w.K * w.T * 8 + w.nseries * w.T * w.M * 4,
+        "trigger (sigma+scan+sort)": w.nseries * (w.T // 16) * 12,
+    }
+    names = list(by_kernel)
+    kernels = []
+    for i, nme in enumerate(names):
+        if kn[i] == 0:
+            continue
+        ms_launch_all = kms[i] / args.steps          # all launches of this kernel in one step
+        kernels.append({"kernel": nme, "launch_groups_per_step": int(kn[i]) // args.steps,
+                        "ms_per_step": ms_launch_all, "share_of_step": ms_launch_all / ms_step,
+                        "algorithmic_GB_per_step": by_kernel[nme] / 1e9,
+                        "achieved_GBps": by_kernel[nme] / 1e9 / (ms_launch_all * 1e-3)})
+    dom = max(kernels, key=lambda k: k["ms_per_step"])
+    chain_bytes = w.input_bytes + w.nseries * w.T * w.M * 4
+    roofline = {"kernel": dom["kernel"], "bound": "hbm", "achieved": dom["achieved_GBps"], "peak": peak,
+                "unit": "GB/s", "frac": dom["achieved_GBps"] / peak, "traffic": None,
+                "peak_source": peak_src,
+                "note": "achieved = algorithmic bytes of all launches of this kernel in a step / their summed "
+                        "CUDA-event time on the launching stream, inside the timed region"}
+    chain = {"algorithmic_GB_per_step": chain_bytes / 1e9,
+             "achieved_GBps": chain_bytes / 1e9 / (ms_step * 1e-3),
+             "frac_of_peak": chain_bytes / 1e9 / (ms_step * 1e-3) / peak,
+             "note": "whole chain: input read once + series written once (SURVEY 8(d) fused count)"}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, cores, sample, dt = oracle_sample(w, X[:, :, :, :2048], tau, 12.0)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt}
+
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic (seeded, paper_1612_06592_b200.synth)",
+        "config": describe(w, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
+        "real_time_factor": value / world / 200e6,
+        "aggregate_samples_per_s_all_series": value * w.nseries,
+        "candidates_last_step": n_cand,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(w.input_bytes),
+                "d2h_bytes_per_step": int(4 + 4 * w.nseries + cap * 24), "ms_per_step": e2e_ms,
+                "real_time_factor": e2e_value / world / 200e6, "steps": e2e_steps,
+                "h2d_GBps": w.input_bytes / 1e9 / (e2e_ms * 1e-3),
+                "api": "lofar_stream_push + lofar_stream_sync (pinned host input, double-buffered)"},
+        "gpu_launches": int(launches),
+        "roofline": roofline, "kernels": kernels, "chain": chain,
+        "cpu_baseline": cpu, "clocks": clocks,
+    }))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json:configs (default 2)")
+    ap.add_argument("--slices", type=int, default=None, help="override slices per block (debugging)")
+    ap.add_argument("--impl", default="gpu", choices=["gpu", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "gpu":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()
