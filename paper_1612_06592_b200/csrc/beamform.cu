@@ -25,63 +25,56 @@ __device__ __forceinline__ float int_to_float_exact(int v)
     return __int_as_float(0x4B400000 + v) - 12582912.0f;
 }
 
-// Load NT complex samples of one (station, pol) row and return them as ints (re, im interleaved).
+// Raw 32-bit words holding NT complex samples of one (station, pol) row.
 template <int NT, bool I16>
-__device__ __forceinline__ void load_row(const void *row, long long t, int nvalid, int *out)
+struct RowWords { static constexpr int value = NT * (I16 ? 4 : 2) / 4; };
+
+template <int NT, bool I16>
+__device__ __forceinline__ void load_raw(const void *row, long long t, int nvalid, int *raw)
 {
+    constexpr int NW = RowWords<NT, I16>::value;
+    const char *p = reinterpret_cast<const char *>(row) + (size_t)t * (I16 ? 4 : 2);
     if (nvalid >= NT) {
-        if constexpr (I16) {
-            const short *p = reinterpret_cast<const short *>(row) + 2 * t;
-            if constexpr (NT == 8) {
-                int4 a = __ldg(reinterpret_cast<const int4 *>(p));
-                int4 b = __ldg(reinterpret_cast<const int4 *>(p) + 1);
-                int w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+        if constexpr (NW >= 4) {
 #pragma unroll
-                for (int i = 0; i < 8; ++i) { out[2 * i] = (short)(w[i] & 0xffff); out[2 * i + 1] = w[i] >> 16; }
-            } else if constexpr (NT == 4) {
-                int4 a = __ldg(reinterpret_cast<const int4 *>(p));
-                int w[4] = {a.x, a.y, a.z, a.w};
-#pragma unroll
-                for (int i = 0; i < 4; ++i) { out[2 * i] = (short)(w[i] & 0xffff); out[2 * i + 1] = w[i] >> 16; }
-            } else {
-                int2 a = __ldg(reinterpret_cast<const int2 *>(p));
-                int w[2] = {a.x, a.y};
-#pragma unroll
-                for (int i = 0; i < 2; ++i) { out[2 * i] = (short)(w[i] & 0xffff); out[2 * i + 1] = w[i] >> 16; }
+            for (int i = 0; i < NW / 4; ++i) {
+                const int4 v = __ldg(reinterpret_cast<const int4 *>(p) + i);
+                raw[4 * i] = v.x; raw[4 * i + 1] = v.y; raw[4 * i + 2] = v.z; raw[4 * i + 3] = v.w;
             }
+        } else if constexpr (NW == 2) {
+            const int2 v = __ldg(reinterpret_cast<const int2 *>(p));
+            raw[0] = v.x; raw[1] = v.y;
         } else {
-            const signed char *p = reinterpret_cast<const signed char *>(row) + 2 * t;
-            if constexpr (NT == 8) {
-                int4 a = __ldg(reinterpret_cast<const int4 *>(p));
-                int w[4] = {a.x, a.y, a.z, a.w};
-#pragma unroll
-                for (int i = 0; i < 16; ++i) out[i] = (signed char)((w[i >> 2] >> (8 * (i & 3))) & 0xff);
-            } else if constexpr (NT == 4) {
-                int2 a = __ldg(reinterpret_cast<const int2 *>(p));
-                int w[2] = {a.x, a.y};
-#pragma unroll
-                for (int i = 0; i < 8; ++i) out[i] = (signed char)((w[i >> 2] >> (8 * (i & 3))) & 0xff);
-            } else {
-                int a = __ldg(reinterpret_cast<const int *>(p));
-#pragma unroll
-                for (int i = 0; i < 4; ++i) out[i] = (signed char)((a >> (8 * i)) & 0xff);
-            }
+            raw[0] = __ldg(reinterpret_cast<const int *>(p));
         }
     } else {
+        // ragged tail: assemble the words from single samples, zero beyond the end of the row
 #pragma unroll
-        for (int i = 0; i < NT; ++i) {
-            int re = 0, im = 0;
-            if (i < nvalid) {
-                if constexpr (I16) {
-                    const short *p = reinterpret_cast<const short *>(row) + 2 * (t + i);
-                    re = p[0]; im = p[1];
-                } else {
-                    const signed char *p = reinterpret_cast<const signed char *>(row) + 2 * (t + i);
-                    re = p[0]; im = p[1];
-                }
-            }
-            out[2 * i] = re; out[2 * i + 1] = im;
+        for (int w = 0; w < NW; ++w) raw[w] = 0;
+        if constexpr (I16) {
+            const unsigned short *q = reinterpret_cast<const unsigned short *>(p);
+#pragma unroll
+            for (int i = 0; i < NT; ++i)
+                if (i < nvalid) raw[i] = (int)((unsigned)q[2 * i] | ((unsigned)q[2 * i + 1] << 16));
+        } else {
+            const unsigned char *q = reinterpret_cast<const unsigned char *>(p);
+#pragma unroll
+            for (int i = 0; i < 2 * NT; ++i)
+                if (i < 2 * nvalid) raw[i >> 2] |= (int)((unsigned)q[i] << (8 * (i & 3)));
         }
+    }
+}
+
+// out[2i], out[2i+1] = re, im of sample i as sign-extended ints.
+template <int NT, bool I16>
+__device__ __forceinline__ void unpack(const int *raw, int *out)
+{
+    if constexpr (I16) {
+#pragma unroll
+        for (int i = 0; i < NT; ++i) { out[2 * i] = (short)(raw[i] & 0xffff); out[2 * i + 1] = raw[i] >> 16; }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 2 * NT; ++i) out[i] = (signed char)((raw[i >> 2] >> (8 * (i & 3))) & 0xff);
     }
 }
 
@@ -114,25 +107,38 @@ __global__ void __launch_bounds__(kBfThreads) beamform_kernel(BeamformArgs a)
 
     const char *Xb = reinterpret_cast<const char *>(a.X);
     const size_t row_bytes = (size_t)a.xpitch * esize;
-#pragma unroll 2
-    for (int s = 0; s < a.S; ++s) {
-        const char *r0 = Xb + ((size_t)(2 * s) * a.K + k) * row_bytes;
-        const char *r1 = Xb + ((size_t)(2 * s + 1) * a.K + k) * row_bytes;
-        int v0[2 * NT], v1[2 * NT];
-        load_row<NT, I16>(r0, t, nvalid, v0);
-        load_row<NT, I16>(r1, t, nvalid, v1);
-        float x[2 * NT];
+    // Stations in groups of G: all 2*G row loads are issued before any of them is used.
+    constexpr int NW = RowWords<NT, I16>::value;
+    constexpr int G = (16 / NW) < 1 ? 1 : ((16 / NW) > 8 ? 8 : (16 / NW));
+    for (int s0 = 0; s0 < a.S; s0 += G) {
+        int raw[G][2][NW];
 #pragma unroll
-        for (int i = 0; i < 2 * NT; ++i) x[i] = int_to_float_exact(v0[i] + v1[i]);
+        for (int g = 0; g < G; ++g) {
+            const int s = (s0 + g < a.S) ? s0 + g : a.S - 1;
+            const char *r0 = Xb + ((size_t)(2 * s) * a.K + k) * row_bytes;
+            load_raw<NT, I16>(r0, t, nvalid, raw[g][0]);
+            load_raw<NT, I16>(r0 + (size_t)a.K * row_bytes, t, nvalid, raw[g][1]);
+        }
 #pragma unroll
-        for (int bb = 0; bb < BT; ++bb) {
-            const float2 w = sW[s * BT + bb];
+        for (int g = 0; g < G; ++g) {
+            if (s0 + g < a.S) {
+                int v0[2 * NT], v1[2 * NT];
+                unpack<NT, I16>(raw[g][0], v0);
+                unpack<NT, I16>(raw[g][1], v1);
+                float x[2 * NT];
 #pragma unroll
-            for (int i = 0; i < NT; ++i) {
-                acc[bb][i].x = fmaf(w.x, x[2 * i], acc[bb][i].x);
-                acc[bb][i].x = fmaf(-w.y, x[2 * i + 1], acc[bb][i].x);
-                acc[bb][i].y = fmaf(w.x, x[2 * i + 1], acc[bb][i].y);
-                acc[bb][i].y = fmaf(w.y, x[2 * i], acc[bb][i].y);
+                for (int i = 0; i < 2 * NT; ++i) x[i] = int_to_float_exact(v0[i] + v1[i]);
+#pragma unroll
+                for (int bb = 0; bb < BT; ++bb) {
+                    const float2 w = sW[(s0 + g) * BT + bb];
+#pragma unroll
+                    for (int i = 0; i < NT; ++i) {
+                        acc[bb][i].x = fmaf(w.x, x[2 * i], acc[bb][i].x);
+                        acc[bb][i].x = fmaf(-w.y, x[2 * i + 1], acc[bb][i].x);
+                        acc[bb][i].y = fmaf(w.x, x[2 * i + 1], acc[bb][i].y);
+                        acc[bb][i].y = fmaf(w.y, x[2 * i], acc[bb][i].y);
+                    }
+                }
             }
         }
     }

@@ -57,24 +57,37 @@ __device__ __forceinline__ float4 load2(const Ctx &c, int k, long long col)
     return v;
 }
 
-// Pre-pass of 16 slices starting at column q into dst[16][kRow].
-__device__ __forceinline__ void prepass(const Ctx &c, long long q, float2 *dst, const float2 *stw, int tid)
+// Global loads of one 16-slice step, held in registers so that they can be issued one step ahead:
+// thread unit i covers conjugate pair m = (tid>>3) + 64 i (m = 0: bins 0 and 256) and slices 2tp, 2tp+1.
+struct StepRegs { float4 a[4], b[4]; };
+
+__device__ __forceinline__ void prefetch(const Ctx &c, long long q, int tid, StepRegs &r)
 {
+    const int tp = tid & 7, m0 = tid >> 3;
+    const long long col = q + 2 * tp;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-        const int u = tid + kThreads * i;
-        const int tp = u & 7, m = u >> 3;
-        const int t = 2 * tp;
-        const long long col = q + t;
-        float2 *r0 = dst + t * kRow, *r1 = r0 + kRow;
+        const int m = m0 + 64 * i;
+        r.a[i] = load2(c, m, col);
+        r.b[i] = load2(c, m == 0 ? 256 : 512 - m, col);
+    }
+}
+
+// Pre-pass of the 16 slices held in r into dst[16][kRow] (packed half-spectrum V, slice-major).
+__device__ __forceinline__ void prepass(const StepRegs &r, float2 *dst, const float2 *stw, int tid)
+{
+    const int tp = tid & 7, m0 = tid >> 3;
+    float2 *r0 = dst + 2 * tp * kRow, *r1 = r0 + kRow;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int m = m0 + 64 * i;
+        const float4 a = r.a[i], b = r.b[i];
         if (m == 0) {
-            const float4 y0 = load2(c, 0, col), y256 = load2(c, 256, col);
-            r0[pad(0)] = prepass_dc(make_float2(y0.x, y0.y));
-            r1[pad(0)] = prepass_dc(make_float2(y0.z, y0.w));
-            r0[pad(256)] = prepass_quarter(make_float2(y256.x, y256.y));
-            r1[pad(256)] = prepass_quarter(make_float2(y256.z, y256.w));
+            r0[pad(0)] = prepass_dc(make_float2(a.x, a.y));
+            r1[pad(0)] = prepass_dc(make_float2(a.z, a.w));
+            r0[pad(256)] = prepass_quarter(make_float2(b.x, b.y));
+            r1[pad(256)] = prepass_quarter(make_float2(b.z, b.w));
         } else {
-            const float4 a = load2(c, m, col), b = load2(c, 512 - m, col);
             const float2 w = stw[m];
             float2 vm, vmir;
             prepass_pair(make_float2(a.x, a.y), make_float2(b.x, b.y), w, vm, vmir);
@@ -155,19 +168,24 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
         __syncthreads();
     } else {
         __syncthreads();   // twiddles visible
-        prepass(c, qs - kStep, cur, stw, tid);
+        StepRegs w;
+        prefetch(c, qs - kStep, tid, w);
+        prepass(w, cur, stw, tid);
         __syncthreads();
         fft512_warp(cur + warp * kRow, stw, lane);
         __syncthreads();
         float2 *t = prev; prev = cur; cur = t;
     }
+    StepRegs regs;
+    prefetch(c, qs, tid, regs);
 
     float *out = a.series ? a.series + (size_t)series * a.series_pitch + a.out0 : nullptr;
     double dsum = 0.0;
 
     for (long long q = qs; q < qe; q += kStep) {
         const int nvalid = (qe - q < kStep) ? (int)(qe - q) : kStep;
-        prepass(c, q, cur, stw, tid);
+        prepass(regs, cur, stw, tid);
+        if (q + kStep < qe) prefetch(c, q + kStep, tid, regs);   // next step's loads fly during FFT + FIR
         __syncthreads();
         fft512_warp(cur + warp * kRow, stw, lane);
         __syncthreads();
