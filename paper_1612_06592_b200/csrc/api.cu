@@ -45,6 +45,7 @@ void dev_free(T *&ptr)
 
 void free_tables(lofar_plan *p)
 {
+    dev_free(p->dWimg);
     dev_free(p->dW); dev_free(p->dDph); dev_free(p->dGs); dev_free(p->dTw);
     dev_free(p->dHist[0]); dev_free(p->dHist[1]); dev_free(p->dTail);
     dev_free(p->dZ); dev_free(p->dPartial); dev_free(p->dChunkMax);
@@ -115,13 +116,23 @@ lofar_status build(lofar_plan *p)
 
     // ---- tables, in double on the host, rounded once to fp32 ----
     std::vector<float2> W((size_t)K * B * S), Dph((size_t)D * K), gs((size_t)kTaps * kHalf), tw(256 + 56 + 448);
+    const bool tc = p->dtype == LOFAR_CI8 && S <= 32 && B <= 128;
+    const size_t img = tc ? tc_image_halfs(S, B) : 0;
+    std::vector<unsigned short> wimg((size_t)K * 2 * img);
+    std::vector<double> wre((size_t)B * S), wim((size_t)B * S);
     for (int j = 0; j < K; ++j) {
         const double f = p->f_zone + (double)(p->k0 + j) * (p->clock / kMfft);
         for (int d = 0; d < D; ++d) Dph[(size_t)d * K + j] = unit_phasor(-(kDispersion * p->stec[d] / f));
         const double fold = (D == 1) ? -(kDispersion * p->stec[0] / f) : 0.0;   // one trial: fold the phase into W
         for (int b = 0; b < B; ++b)
-            for (int s = 0; s < S; ++s)
-                W[((size_t)j * B + b) * S + s] = unit_phasor(f * p->tau[(size_t)b * S + s] + (fold - std::floor(fold)));
+            for (int s = 0; s < S; ++s) {
+                double turns = f * p->tau[(size_t)b * S + s] + (fold - std::floor(fold));
+                turns -= std::floor(turns);
+                W[((size_t)j * B + b) * S + s] = unit_phasor(turns);
+                wre[(size_t)b * S + s] = std::cos(kTwoPi * turns);
+                wim[(size_t)b * S + s] = std::sin(kTwoPi * turns);
+            }
+        if (tc) tc_build_image(wre.data(), wim.data(), S, B, &wimg[(size_t)j * 2 * img], &wimg[((size_t)j * 2 + 1) * img]);
     }
     for (int t = 0; t < kTaps; ++t)
         for (int n = 0; n < kHalf; ++n)
@@ -138,6 +149,10 @@ lofar_status build(lofar_plan *p)
     if ((st = dev_alloc(p, &p->dDph, Dph.size())) != LOFAR_OK) return st;
     if ((st = dev_alloc(p, &p->dGs, gs.size())) != LOFAR_OK) return st;
     if ((st = dev_alloc(p, &p->dTw, tw.size())) != LOFAR_OK) return st;
+    if (tc) {
+        if ((st = dev_alloc(p, &p->dWimg, wimg.size())) != LOFAR_OK) return st;
+        CU(cudaMemcpy(p->dWimg, wimg.data(), wimg.size() * sizeof(unsigned short), cudaMemcpyHostToDevice));
+    }
     CU(cudaMemcpy(p->dW, W.data(), W.size() * sizeof(float2), cudaMemcpyHostToDevice));
     CU(cudaMemcpy(p->dDph, Dph.data(), Dph.size() * sizeof(float2), cudaMemcpyHostToDevice));
     CU(cudaMemcpy(p->dGs, gs.data(), gs.size() * sizeof(float2), cudaMemcpyHostToDevice));
@@ -197,6 +212,12 @@ void plan_spans(long long nsteps, int nseries, int sms, int *nspans, int *span_l
     const long long per = (nsteps + best - 1) / best;
     *nspans = (int)((nsteps + per - 1) / per);
     *span_len = (int)(per * kStepSlices);
+}
+
+int beamform_dispatch(lofar_plan *p, const BeamformArgs &b, cudaStream_t st)
+{
+    if (p->dWimg && p->B >= p->tc_min_beams && tc_supported(b)) return launch_beamform_tc(b, p->dWimg, st);
+    return launch_beamform(b, st);
 }
 
 lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, long long nc, int zmap_trials,
@@ -261,7 +282,7 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
         b.S = p->S; b.K = p->K; b.B = p->B; b.nphase = 0; b.dtype = p->dtype;
         {
             ProfScope prof(p, 0, st);
-            const int n = launch_beamform(b, st);
+            const int n = beamform_dispatch(p, b, st);
             if (n < 0) return LOFAR_E_CUDA;
             p->launches += n;
         }
@@ -414,7 +435,7 @@ lofar_status lofar_beamform_dedisperse(lofar_plan *p, const void *X, int slices,
     b.W = p->dW; b.Dph = p->dDph;
     b.S = p->S; b.K = p->K; b.B = p->B; b.nphase = p->D > 1 ? p->D : 0; b.dtype = p->dtype;
     ProfScope prof(p, 0, static_cast<cudaStream_t>(stream));
-    const int n = launch_beamform(b, static_cast<cudaStream_t>(stream));
+    const int n = beamform_dispatch(p, b, static_cast<cudaStream_t>(stream));
     if (n < 0) return LOFAR_E_CUDA;
     p->launches += n;
     return LOFAR_OK;

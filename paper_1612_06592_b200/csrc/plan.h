@@ -67,6 +67,11 @@ struct TriggerArgs {
 // kernel launchers (each returns the number of kernels it launched, or -1 on a launch error)
 int launch_beamform(const BeamformArgs &a, cudaStream_t st);
 int launch_ippf(const IppfArgs &a, cudaStream_t st);
+// tensor-core beamformer (beamform_tc.cu)
+bool tc_supported(const BeamformArgs &a);
+size_t tc_image_halfs(int S, int B);
+void tc_build_image(const double *w_re, const double *w_im, int S, int B, unsigned short *hi, unsigned short *lo);
+int launch_beamform_tc(const BeamformArgs &a, const void *wimg, cudaStream_t st);
 int ippf_configure();                                   // opt in to the large dynamic shared memory
 int launch_trigger_reduce(const TriggerArgs &a, cudaStream_t st);   // sum e^2 + chunk max from the series
 int launch_trigger_finish(const TriggerArgs &a, cudaStream_t st);   // sigma, threshold scan, sort
@@ -88,6 +93,8 @@ struct lofar_plan {
     // device state
     bool built = false;
     int num_sms = 148;
+    unsigned short *dWimg = nullptr;   // [K][2][image] fp16 hi/lo operand images for the tensor-core beamformer
+    int tc_min_beams = 4;              // use tcgen05 from this many beams on (int8 input)
     float2 *dW = nullptr, *dDph = nullptr, *dGs = nullptr, *dTw = nullptr;
     float *dHist[2] = {nullptr, nullptr};
     int hist_parity = 0;
