@@ -65,11 +65,26 @@ __device__ __forceinline__ void prefetch(const Ctx &c, long long q, int tid, Ste
 {
     const int tp = tid & 7, m0 = tid >> 3;
     const long long col = q + 2 * tp;
+    if (c.vec_ok && col + 1 < c.nc && c.ph == nullptr) {
+        // common case, branch-free: predicated 16-byte loads, rows outside the selected band read as zero
+        const float2 *p0 = c.Zs + col;
+        const unsigned K = (unsigned)c.K, zp = (unsigned)c.zpitch;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int m = m0 + 64 * i;
-        r.a[i] = load2(c, m, col);
-        r.b[i] = load2(c, m == 0 ? 256 : 512 - m, col);
+        for (int i = 0; i < 4; ++i) {
+            const int m = m0 + 64 * i;
+            const unsigned ja = (unsigned)(m - c.k0), jb = (unsigned)((m == 0 ? 256 : 512 - m) - c.k0);
+            float4 va = make_float4(0.f, 0.f, 0.f, 0.f), vb = va;
+            if (ja < K) va = __ldcs(reinterpret_cast<const float4 *>(p0 + (size_t)(ja * zp)));
+            if (jb < K) vb = __ldcs(reinterpret_cast<const float4 *>(p0 + (size_t)(jb * zp)));
+            r.a[i] = va; r.b[i] = vb;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int m = m0 + 64 * i;
+            r.a[i] = load2(c, m, col);
+            r.b[i] = load2(c, m == 0 ? 256 : 512 - m, col);
+        }
     }
 }
 
