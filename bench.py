@@ -146,6 +146,24 @@ def run_reference(args):
     }))
 
 
+# ------------------------------------------------------------------------------------- replicas
+def max_over_ranks(value: float, dist, device="cpu") -> float:
+    """MAX over ranks of a per-rank duration (the contract's multi-GPU timing rule).  The path has no
+    sharding or collectives (north_star: "replicas only"), so this and the barrier are the only
+    cross-rank operations in the bench."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(samples_per_block: int, world: int, ms_step_max: float) -> float:
+    """Whole-job samples/s per beam: every replica reconstructs its own block per step."""
+    return world * samples_per_block / (ms_step_max * 1e-3)
+
+
 # ------------------------------------------------------------------------------------- GPU arm
 def run_gpu(args):
     import torch
@@ -198,10 +216,7 @@ def run_gpu(args):
     launches = plan.launch_count() - l0
     kms, kn = plan.profile_read()
     plan.profile(False)
-    if dist is not None:
-        t = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, "cuda")
     ms_step = ms_total / args.steps
     n_cand = int(count.item())
 
@@ -222,10 +237,7 @@ def run_gpu(args):
     plan.stream_sync()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dist, "cuda")
     e2e_ms = e2e_s / e2e_steps * 1e3
 
     if rank != 0:
@@ -234,8 +246,8 @@ def run_gpu(args):
         return
 
     samples_per_block = w.T * w.M
-    value = world * samples_per_block / (ms_step * 1e-3)            # per beam, all replicas
-    e2e_value = world * samples_per_block / (e2e_ms * 1e-3)
+    value = aggregate_value(samples_per_block, world, ms_step)       # per beam, all replicas
+    e2e_value = aggregate_value(samples_per_block, world, e2e_ms)
     peak, peak_src = peaks()
 
     # algorithmic bytes per launch
@@ -246,23 +258,36 @@ def run_gpu(args):
         "ippf_kernel": zrows * w.K * w.T * 8 + w.nseries * w.T * w.M * 4,
         "trigger (sigma+scan+sort)": w.nseries * (w.T // 16) * 12,
     }
+    tc = w.dtype == "ci8" and w.B >= 4 and w.S <= 32
     names = list(by_kernel)
+    shown = {"beamform_kernel": "beamform_tc_kernel" if tc else "beamform_kernel"}
     kernels = []
     for i, nme in enumerate(names):
         if kn[i] == 0:
             continue
         ms_launch_all = kms[i] / args.steps          # all launches of this kernel in one step
-        kernels.append({"kernel": nme, "launch_groups_per_step": int(kn[i]) // args.steps,
-                        "ms_per_step": ms_launch_all, "share_of_step": ms_launch_all / ms_step,
-                        "algorithmic_GB_per_step": by_kernel[nme] / 1e9,
+        per_step = int(kn[i]) // args.steps
+        kernels.append({"kernel": shown.get(nme, nme), "launches_per_step": per_step,
+                        "ms_per_step": ms_launch_all, "ms_per_launch": ms_launch_all / per_step,
+                        "share_of_step": ms_launch_all / ms_step,
+                        "algorithmic_GB_per_launch": by_kernel[nme] / 1e9 / per_step,
                         "achieved_GBps": by_kernel[nme] / 1e9 / (ms_launch_all * 1e-3)})
     dom = max(kernels, key=lambda k: k["ms_per_step"])
     chain_bytes = w.input_bytes + w.nseries * w.T * w.M * 4
+    # dram__bytes_read.sum + dram__bytes_write.sum over algorithmic bytes of the same launch, from the committed
+    # ncu --set full capture of configs[2] (profiles/r1_c_ncu_full.md); other workloads have no capture yet
+    ncu_ratio = {"ippf_kernel": 8.656201 / 8.650752, "beamform_tc_kernel": 6.289329 / 6.332375}
+    traffic = None
+    if w.index == 2 and args.slices is None and dom["kernel"] in ncu_ratio:
+        traffic = dom["algorithmic_GB_per_launch"] * ncu_ratio[dom["kernel"]]
     roofline = {"kernel": dom["kernel"], "bound": "hbm", "achieved": dom["achieved_GBps"], "peak": peak,
-                "unit": "GB/s", "frac": dom["achieved_GBps"] / peak, "traffic": None,
-                "peak_source": peak_src,
-                "note": "achieved = algorithmic bytes of all launches of this kernel in a step / their summed "
-                        "CUDA-event time on the launching stream, inside the timed region"}
+                "unit": "GB/s", "frac": dom["achieved_GBps"] / peak, "traffic": traffic,
+                "traffic_unit": "GB per launch (ncu dram bytes, profiles/r1_c_ncu_full.md)",
+                "algorithmic_GB_per_launch": dom["algorithmic_GB_per_launch"],
+                "ms_per_launch": dom["ms_per_launch"], "peak_source": peak_src,
+                "note": "achieved = algorithmic bytes per launch / mean launch duration, CUDA events on the "
+                        "launching stream inside the timed region (K*8 B read + 4096 B written per series-slice "
+                        "for ippf_kernel; 2*S*2*esize B read + B*8 B written per (sub-band, slice) for beamform)"}
     chain = {"algorithmic_GB_per_step": chain_bytes / 1e9,
              "achieved_GBps": chain_bytes / 1e9 / (ms_step * 1e-3),
              "frac_of_peak": chain_bytes / 1e9 / (ms_step * 1e-3) / peak,
