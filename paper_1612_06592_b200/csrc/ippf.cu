@@ -212,6 +212,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 #pragma unroll
         for (int j = 0; j < kStep; ++j) acc[j] = make_float2(0.f, 0.f);
         const int pn = pad(tid);
+        float ssum = 0.f, smax = 0.f;
 #pragma unroll
         for (int i = 0; i < kP - 1 + kStep; ++i) {
             const float2 x = (i < kP - 1) ? prev[(i + 1) * kRow + pn] : cur[(i - (kP - 1)) * kRow + pn];
@@ -223,15 +224,16 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
                     acc[j].y = fmaf(g[t].y, x.y, acc[j].y);
                 }
             }
-        }
-        float ssum = 0.f, smax = 0.f;
-#pragma unroll
-        for (int j = 0; j < kStep; ++j) {
-            if (j < nvalid) {
-                if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)(q + j) * kM + 2 * tid), acc[j]);
-                ssum = fmaf(acc[j].x, acc[j].x, ssum);
-                ssum = fmaf(acc[j].y, acc[j].y, ssum);
-                smax = fmaxf(smax, fmaxf(fabsf(acc[j].x), fabsf(acc[j].y)));
+            // output slice j = i - 15 is complete once window element i has been applied: store it now so
+            // that the 64 KB of stores per step are spread over the second half of the FIR
+            if (i >= kP - 1) {
+                const int j = i - (kP - 1);
+                if (j < nvalid) {
+                    if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)(q + j) * kM + 2 * tid), acc[j]);
+                    ssum = fmaf(acc[j].x, acc[j].x, ssum);
+                    ssum = fmaf(acc[j].y, acc[j].y, ssum);
+                    smax = fmaxf(smax, fmaxf(fabsf(acc[j].x), fabsf(acc[j].y)));
+                }
             }
         }
         dsum += (double)ssum;
