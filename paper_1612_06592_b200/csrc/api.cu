@@ -176,7 +176,7 @@ lofar_status build(lofar_plan *p)
     long long zc = (long long)(kScratchBudget / ((size_t)B * K * sizeof(float2)));
     zc = zc / 1024 * 1024;
     if (zc < 1024) zc = 1024;
-    p->zchunk = zc < cap ? zc : cap;
+    p->zchunk = round_up(zc < cap ? zc : cap, 32);      // whole 32-slice tiles of the scratch layout
     if ((st = dev_alloc(p, &p->dZ, (size_t)B * K * p->zchunk)) != LOFAR_OK) return st;
     const long long nsteps = cap / kStepSlices;
     p->partial_pitch = (int)nsteps;
@@ -220,12 +220,12 @@ int beamform_dispatch(lofar_plan *p, const BeamformArgs &b, cudaStream_t st)
     return launch_beamform(b, st);
 }
 
-lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, long long nc, int zmap_trials,
+lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, int ztile, long long nc, int zmap_trials,
                      float *series, long long series_pitch, long long out0, int *partial0, long long step0,
                      cudaStream_t st)
 {
     IppfArgs a{};
-    a.Z = Z; a.zpitch = zpitch; a.nc = nc;
+    a.Z = Z; a.zpitch = zpitch; a.ztile = ztile; a.nc = nc;
     a.series = series; a.series_pitch = series_pitch; a.out0 = out0;
     a.Dph = p->dDph; a.zmap_trials = zmap_trials;
     a.K = p->K; a.k0 = p->k0; a.nseries = p->B * p->D;
@@ -278,7 +278,7 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
         const long long nc = (T - c0 < p->zchunk) ? T - c0 : p->zchunk;
         BeamformArgs b{};
         b.X = X; b.xpitch = T; b.t0 = c0; b.nt = nc;
-        b.Z = p->dZ; b.zpitch = p->zchunk;
+        b.Z = p->dZ; b.zpitch = p->zchunk; b.ztile = 1;
         b.W = p->dW; b.Dph = p->dDph;
         b.S = p->S; b.K = p->K; b.B = p->B; b.nphase = 0; b.dtype = p->dtype;
         {
@@ -287,7 +287,7 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
             if (n < 0) return LOFAR_E_CUDA;
             p->launches += n;
         }
-        lofar_status s = do_ippf(p, p->dZ, p->zchunk, nc, p->D > 1 ? p->D : 0, series, N, c0 * kMfft, &partial0,
+        lofar_status s = do_ippf(p, p->dZ, p->zchunk, 1, nc, p->D > 1 ? p->D : 0, series, N, c0 * kMfft, &partial0,
                                  c0 / kStepSlices, st);
         if (s != LOFAR_OK) return s;
     }
@@ -413,7 +413,7 @@ lofar_status lofar_plan_workspace_bytes(lofar_plan *p, size_t *bytes)
     const long long cap = round_up(p->max_slices > 0 ? p->max_slices : kStepSlices, kStepSlices);
     long long zc = (long long)(kScratchBudget / ((size_t)p->B * p->K * sizeof(float2))) / 1024 * 1024;
     if (zc < 1024) zc = 1024;
-    if (zc > cap) zc = cap;
+    if (zc > cap) zc = round_up(cap, 32);
     size_t b = 0;
     b += ((size_t)p->K * p->B * p->S + (size_t)p->D * p->K + (size_t)kTaps * kHalf + 760) * sizeof(float2);
     b += 2 * ns * (kTaps - 1) * kMfft * sizeof(float);
@@ -432,7 +432,7 @@ lofar_status lofar_beamform_dedisperse(lofar_plan *p, const void *X, int slices,
     if ((s = check_x(p, X, slices)) != LOFAR_OK) return s;
     BeamformArgs b{};
     b.X = X; b.xpitch = slices; b.t0 = 0; b.nt = slices;
-    b.Z = static_cast<float2 *>(Z); b.zpitch = slices;
+    b.Z = static_cast<float2 *>(Z); b.zpitch = slices; b.ztile = 0;
     b.W = p->dW; b.Dph = p->dDph;
     b.S = p->S; b.K = p->K; b.B = p->B; b.nphase = p->D > 1 ? p->D : 0; b.dtype = p->dtype;
     ProfScope prof(p, 0, static_cast<cudaStream_t>(stream));
@@ -449,7 +449,7 @@ lofar_status lofar_inverse_ppf(lofar_plan *p, const void *Z, int slices, float *
     if (!Z || !series) return LOFAR_E_INVALID;
     if (reinterpret_cast<size_t>(Z) & 7 || reinterpret_cast<size_t>(series) & 7) return LOFAR_E_ALIGN;
     int partial0 = 0;
-    return do_ippf(p, static_cast<const float2 *>(Z), slices, slices, 0, series, (long long)slices * kMfft, 0,
+    return do_ippf(p, static_cast<const float2 *>(Z), slices, 0, slices, 0, series, (long long)slices * kMfft, 0,
                    &partial0, 0, static_cast<cudaStream_t>(stream));
 }
 

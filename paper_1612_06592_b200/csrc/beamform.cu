@@ -160,7 +160,8 @@ __global__ void __launch_bounds__(kBfThreads) beamform_kernel(BeamformArgs a)
 #pragma unroll
                 for (int i = 0; i < NT; ++i) o[i] = acc[bb][i];
             }
-            float2 *zr = a.Z + ((size_t)((b0 + bb) * nph + d) * a.K + k) * (size_t)a.zpitch + col;
+            float2 *zr = a.Z + (size_t)((b0 + bb) * nph + d) * a.K * (size_t)a.zpitch +
+                         (a.ztile ? ((size_t)(col >> 5) * a.K + k) * 32 + (col & 31) : (size_t)k * a.zpitch + col);
             if (vec) {
 #pragma unroll
                 for (int i = 0; i < NT; i += 2)

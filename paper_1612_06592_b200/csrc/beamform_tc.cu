@@ -195,7 +195,9 @@ __global__ void __launch_bounds__(kTcThreads) beamform_tc_kernel(TcArgs a)
                 for (int j = 0; j < 8; ++j) {
                     const int b = n0 / 2 + j;
                     if (b < g.B) {
-                        float2 *zr = g.Z + ((size_t)b * g.K + k) * (size_t)g.zpitch + colt;
+                        float2 *zr = g.Z + (size_t)b * g.K * (size_t)g.zpitch +
+                                     (g.ztile ? ((size_t)(colt >> 5) * g.K + k) * 32 + (colt & 31)
+                                              : (size_t)k * g.zpitch + colt);
                         *zr = make_float2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
                     }
                 }

@@ -29,7 +29,7 @@ struct Ctx {
     const float2 *Zs;      // rows of this series' beam (sub-band j at Zs + j*zpitch)
     const float2 *ph;      // trial phasors of this series or nullptr
     long long zpitch, nc;
-    int K, k0, vec_ok;
+    int K, k0, vec_ok, tiled;
 };
 
 // Two consecutive slices (col, col+1) of absolute sub-band k; zero outside the selected band / launch.
@@ -38,7 +38,8 @@ __device__ __forceinline__ float4 load2(const Ctx &c, int k, long long col)
     const int j = k - c.k0;
     float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
     if (j < 0 || j >= c.K || col >= c.nc) return v;
-    const float2 *p = c.Zs + (size_t)j * c.zpitch + col;
+    const float2 *p = c.tiled ? c.Zs + ((size_t)(col >> 5) * c.K + j) * 32 + (col & 31)
+                              : c.Zs + (size_t)j * c.zpitch + col;
     if (col + 1 < c.nc) {
         if (c.vec_ok) {
             v = __ldcs(reinterpret_cast<const float4 *>(p));
@@ -67,8 +68,9 @@ __device__ __forceinline__ void prefetch(const Ctx &c, long long q, int tid, Ste
     const long long col = q + 2 * tp;
     if (c.vec_ok && col + 1 < c.nc && c.ph == nullptr) {
         // common case, branch-free: predicated 16-byte loads, rows outside the selected band read as zero
-        const float2 *p0 = c.Zs + col;
-        const unsigned K = (unsigned)c.K, zp = (unsigned)c.zpitch;
+        // tiled scratch: 32-slice tiles [K][32]: a step reads 128 of every 256 bytes of one contiguous block; else rows zpitch apart
+        const float2 *p0 = c.tiled ? c.Zs + (size_t)(col >> 5) * c.K * 32 + (col & 31) : c.Zs + col;
+        const unsigned K = (unsigned)c.K, zp = c.tiled ? 32u : (unsigned)c.zpitch;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int m = m0 + 64 * i;
@@ -169,7 +171,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     const int zi = a.zmap_trials ? series / a.zmap_trials : series;
     c.Zs = a.Z + (size_t)zi * a.K * (size_t)a.zpitch;
     c.ph = a.zmap_trials ? a.Dph + (size_t)(series % a.zmap_trials) * a.K : nullptr;
-    c.zpitch = a.zpitch; c.nc = a.nc; c.K = a.K; c.k0 = a.k0; c.vec_ok = a.vec_ok;
+    c.zpitch = a.zpitch; c.nc = a.nc; c.K = a.K; c.k0 = a.k0; c.vec_ok = a.vec_ok; c.tiled = a.ztile;
 
     for (int i = tid; i < kP * kH; i += kThreads) sg[i] = a.gs[i];
     for (int i = tid; i < kTwCount; i += kThreads) stw[i] = a.tw[i];

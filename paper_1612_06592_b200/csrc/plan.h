@@ -17,6 +17,7 @@ struct BeamformArgs {
     long long nt;         // slices to process
     float2 *Z;            // [nz][K][zpitch], slice t0+i stored at column i
     long long zpitch;
+    int ztile;            // 1: plan scratch layout [nz][zpitch/32][K][32] (32-slice tiles contiguous over sub-bands)
     const float2 *W;      // [K][B][S] weights (de-dispersion phase folded in when D == 1)
     const float2 *Dph;    // [D][K] trial phasors, used when nphase > 0
     int S, K, B;
@@ -27,6 +28,7 @@ struct BeamformArgs {
 struct IppfArgs {
     const float2 *Z;      // [nz][K][zpitch]
     long long zpitch;
+    int ztile;            // 1: [nz][zpitch/32][K][32]
     long long nc;         // slices in this launch (columns 0..nc-1 of Z)
     float *series;        // [nseries][series_pitch]; this launch writes samples out0 .. out0 + nc*1024
     long long series_pitch;
