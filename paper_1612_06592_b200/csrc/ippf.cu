@@ -221,10 +221,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 #pragma unroll
             for (int t = 0; t < kP; ++t) {
                 const int j = i - (kP - 1) + t;
-                if (j >= 0 && j < kStep) {
-                    acc[j].x = fmaf(g[t].x, x.x, acc[j].x);
-                    acc[j].y = fmaf(g[t].y, x.y, acc[j].y);
-                }
+                if (j >= 0 && j < kStep) acc[j] = fma2(g[t], x, acc[j]);
             }
             // output slice j = i - 15 is complete once window element i has been applied: store it now so
             // that the 64 KB of stores per step are spread over the second half of the FIR
