@@ -51,10 +51,6 @@ __device__ __forceinline__ float4 load2(const Ctx &c, int k, long long col)
         float2 z0 = p[0];
         v.x = z0.x; v.y = z0.y;
     }
-    if (c.ph) {
-        const float2 f = c.ph[j];
-        v = make_float4(f.x * v.x - f.y * v.y, f.x * v.y + f.y * v.x, f.x * v.z - f.y * v.w, f.x * v.w + f.y * v.z);
-    }
     return v;
 }
 
@@ -66,7 +62,7 @@ __device__ __forceinline__ void prefetch(const Ctx &c, long long q, int tid, Ste
 {
     const int tp = tid & 7, m0 = tid >> 3;
     const long long col = q + 2 * tp;
-    if (c.vec_ok && col + 1 < c.nc && c.ph == nullptr) {
+    if (c.vec_ok && col + 1 < c.nc) {
         // common case, branch-free: predicated 16-byte loads, rows outside the selected band read as zero
         // tiled scratch: 32-slice tiles [K][32]: a step reads 128 of every 256 bytes of one contiguous block; else rows zpitch apart
         const float2 *p0 = c.tiled ? c.Zs + (size_t)(col >> 5) * c.K * 32 + (col & 31) : c.Zs + col;
@@ -91,14 +87,25 @@ __device__ __forceinline__ void prefetch(const Ctx &c, long long q, int tid, Ste
 }
 
 // Pre-pass of the 16 slices held in r into dst[16][kRow] (packed half-spectrum V, slice-major).
-__device__ __forceinline__ void prepass(const StepRegs &r, float2 *dst, const float2 *stw, int tid)
+__device__ __forceinline__ float4 rotate2(float4 v, float2 f)
+{
+    return make_float4(f.x * v.x - f.y * v.y, f.x * v.y + f.y * v.x, f.x * v.z - f.y * v.w, f.x * v.w + f.y * v.z);
+}
+
+__device__ __forceinline__ void prepass(const Ctx &c, const StepRegs &r, float2 *dst, const float2 *stw, int tid)
 {
     const int tp = tid & 7, m0 = tid >> 3;
     float2 *r0 = dst + 2 * tp * kRow, *r1 = r0 + kRow;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int m = m0 + 64 * i;
-        const float4 a = r.a[i], b = r.b[i];
+        float4 a = r.a[i], b = r.b[i];
+        if (c.ph) {
+            // STEC trial fan-out (a2): the trial's phasor multiplies the beam sums as they enter the transform
+            const unsigned ja = (unsigned)(m - c.k0), jb = (unsigned)((m == 0 ? 256 : 512 - m) - c.k0);
+            if (ja < (unsigned)c.K) a = rotate2(a, __ldg(c.ph + ja));
+            if (jb < (unsigned)c.K) b = rotate2(b, __ldg(c.ph + jb));
+        }
         if (m == 0) {
             r0[pad(0)] = prepass_dc(make_float2(a.x, a.y));
             r1[pad(0)] = prepass_dc(make_float2(a.z, a.w));
@@ -187,7 +194,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
         __syncthreads();   // twiddles visible
         StepRegs w;
         prefetch(c, qs - kStep, tid, w);
-        prepass(w, cur, stw, tid);
+        prepass(c, w, cur, stw, tid);
         __syncthreads();
         fft512_warp(cur + warp * kRow, stw, lane);
         __syncthreads();
@@ -201,7 +208,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 
     for (long long q = qs; q < qe; q += kStep) {
         const int nvalid = (qe - q < kStep) ? (int)(qe - q) : kStep;
-        prepass(regs, cur, stw, tid);
+        prepass(c, regs, cur, stw, tid);
         if (q + kStep < qe) prefetch(c, q + kStep, tid, regs);   // next step's loads fly during FFT + FIR
         __syncthreads();
         fft512_warp(cur + warp * kRow, stw, lane);
