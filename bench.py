@@ -293,6 +293,29 @@ def run_gpu(args):
              "frac_of_peak": chain_bytes / 1e9 / (ms_step * 1e-3) / peak,
              "note": "whole chain: input read once + series written once (SURVEY 8(d) fused count)"}
 
+    # cuFFT (through torch.fft.irfft), timed ONLY as a comparison for step a3 (north_star); never on the product path.
+    cufft = None
+    if args.compare_cufft and world == 1:
+        nb = min(w.nseries * w.T, 1 << 19)                       # slices per batch (4 GB of spectra + 2 GB out)
+        spec = torch.zeros((nb, 513), dtype=torch.complex64, device="cuda")
+        spec[:, w.k0:w.k0 + w.K] = torch.randn((nb, w.K), dtype=torch.complex64, device="cuda")
+        for _ in range(2):
+            y = torch.fft.irfft(spec, n=1024, dim=1, norm="forward")
+        torch.cuda.synchronize()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record()
+        for _ in range(5):
+            y = torch.fft.irfft(spec, n=1024, dim=1, norm="forward")
+        c1.record()
+        torch.cuda.synchronize()
+        ms = c0.elapsed_time(c1) / 5
+        cufft = {"what": "torch.fft.irfft (cuFFT C2R, 1024 points) on dense 513-bin spectra already transposed to "
+                         "slice-major; no beam-sum transpose, no FIR, no trigger sums", "slices": nb,
+                 "ns_per_slice": ms * 1e6 / nb, "ms_scaled_to_block": ms * (w.nseries * w.T) / nb,
+                 "ippf_kernel_ns_per_slice": next(k["ms_per_step"] for k in kernels if k["kernel"] == "ippf_kernel")
+                 * 1e6 / (w.nseries * w.T)}
+        del spec, y
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         v, cores, sample, dt = oracle_sample(w, X[:, :, :, :2048], tau, 12.0)
@@ -314,7 +337,7 @@ def run_gpu(args):
                 "api": "lofar_stream_push + lofar_stream_sync (pinned host input, double-buffered)"},
         "gpu_launches": int(launches),
         "roofline": roofline, "kernels": kernels, "chain": chain,
-        "cpu_baseline": cpu, "clocks": clocks,
+        "cpu_baseline": cpu, "clocks": clocks, "cufft_comparison": cufft,
     }))
     if dist is not None:
         dist.destroy_process_group()
@@ -329,6 +352,7 @@ def main():
     ap.add_argument("--slices", type=int, default=None, help="override slices per block (debugging)")
     ap.add_argument("--impl", default="gpu", choices=["gpu", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--compare-cufft", action="store_true", help="also time cuFFT C2R (via torch) as a comparison for a3")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "gpu":
         args.warmup = 3
