@@ -76,6 +76,17 @@ __device__ __forceinline__ void prefetch(const Ctx &c, long long q, int tid, Ste
             if (jb < K) vb = __ldcs(reinterpret_cast<const float4 *>(p0 + (size_t)(jb * zp)));
             r.a[i] = va; r.b[i] = vb;
         }
+        // pull the rows of the step after this one into L2 (one 128-byte line per row: lanes with tp == 0)
+        if (tp == 0 && col + 2 * kStep < c.nc) {
+            const float2 *p1 = c.tiled ? c.Zs + (size_t)((col + kStep) >> 5) * c.K * 32 + ((col + kStep) & 31) : p0 + kStep;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int m = m0 + 64 * i;
+                const unsigned ja = (unsigned)(m - c.k0), jb = (unsigned)((m == 0 ? 256 : 512 - m) - c.k0);
+                if (ja < K) asm volatile("prefetch.global.L2 [%0];" :: "l"(p1 + (size_t)(ja * zp)));
+                if (jb < K) asm volatile("prefetch.global.L2 [%0];" :: "l"(p1 + (size_t)(jb * zp)));
+            }
+        }
     } else {
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -228,7 +239,10 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 #pragma unroll
             for (int t = 0; t < kP; ++t) {
                 const int j = i - (kP - 1) + t;
-                if (j >= 0 && j < kStep) acc[j] = fma2(g[t], x, acc[j]);
+                if (j >= 0 && j < kStep) {
+                    acc[j].x = fmaf(g[t].x, x.x, acc[j].x);
+                    acc[j].y = fmaf(g[t].y, x.y, acc[j].y);
+                }
             }
             // output slice j = i - 15 is complete once window element i has been applied: store it now so
             // that the 64 KB of stores per step are spread over the second half of the FIR
