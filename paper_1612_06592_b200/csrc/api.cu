@@ -115,7 +115,7 @@ lofar_status build(lofar_plan *p)
     const int S = p->S, K = p->K, B = p->B, D = p->D, ns = B * D;
 
     // ---- tables, in double on the host, rounded once to fp32 ----
-    std::vector<float2> W((size_t)K * B * S), Dph((size_t)D * K), gs((size_t)kTaps * kHalf), tw(256 + 56 + 448);
+    std::vector<float2> W((size_t)K * B * S), Dph((size_t)D * K), gs((size_t)kTaps * kHalf), tw(256 + 512);
     const bool tc = p->dtype == LOFAR_CI8 && S <= 32 && B <= 128;
     const size_t img = tc ? tc_image_halfs(S, B) : 0;
     std::vector<unsigned short> wimg((size_t)K * 2 * img);
@@ -138,11 +138,10 @@ lofar_status build(lofar_plan *p)
         for (int n = 0; n < kHalf; ++n)
             gs[(size_t)t * kHalf + n] = make_float2((float)(kMfft * p->h[2 * n + kMfft * t]),
                                                     (float)(kMfft * p->h[2 * n + 1 + kMfft * t]));
+    // twiddles: w1024[256] for the pre-pass, TB[r][j] = exp(2 pi i j r / 512) (r < 32, j < 16) for the radix-32 pass
     for (int m = 0; m < 256; ++m) tw[m] = unit_phasor((double)m / 1024.0);
-    for (int r = 1; r < 8; ++r) {
-        for (int jj = 0; jj < 8; ++jj) tw[256 + (r - 1) * 8 + jj] = unit_phasor((double)(jj * r) / 64.0);
-        for (int jj = 0; jj < 64; ++jj) tw[312 + (r - 1) * 64 + jj] = unit_phasor((double)(jj * r) / 512.0);
-    }
+    for (int r = 0; r < 32; ++r)
+        for (int jj = 0; jj < 16; ++jj) tw[256 + r * 16 + jj] = unit_phasor((double)(jj * r) / 512.0);
 
     lofar_status st;
     if ((st = dev_alloc(p, &p->dW, W.size())) != LOFAR_OK) return st;
@@ -415,7 +414,7 @@ lofar_status lofar_plan_workspace_bytes(lofar_plan *p, size_t *bytes)
     if (zc < 1024) zc = 1024;
     if (zc > cap) zc = round_up(cap, 32);
     size_t b = 0;
-    b += ((size_t)p->K * p->B * p->S + (size_t)p->D * p->K + (size_t)kTaps * kHalf + 760) * sizeof(float2);
+    b += ((size_t)p->K * p->B * p->S + (size_t)p->D * p->K + (size_t)kTaps * kHalf + 768) * sizeof(float2);
     b += 2 * ns * (kTaps - 1) * kMfft * sizeof(float);
     b += ns * (size_t)(p->env_window - 1) * sizeof(float);
     b += (size_t)p->B * p->K * zc * sizeof(float2);

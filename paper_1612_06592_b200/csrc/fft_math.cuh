@@ -2,7 +2,7 @@
 // (step a3, "an inverse Fourier transformation F^-1 y~ = y").
 //
 // The 1024-point Hermitian inverse transform of one time slice is computed as one 512-point
-// complex inverse FFT (three Stockham radix-8 passes) of
+// complex inverse FFT (a radix-16 pass and a radix-32 pass, one shared-memory exchange between them) of
 //     V[k] = (Y[k] + conj(Y[512-k])) + i w^k (Y[k] - conj(Y[512-k])),   w = exp(2 pi i / 1024),
 // whose output v[n] = y[2n] + i y[2n+1] is the real series in natural order.
 // Everything here is __host__ __device__ so that the index logic can be exercised on the CPU
@@ -67,6 +67,25 @@ LOFAR_HD void idft8(float2 *x)
     x[1] = cadd(e1, t1); x[5] = csub(e1, t1);
     x[2] = cadd(e2, t2); x[6] = csub(e2, t2);
     x[3] = cadd(e3, t3); x[7] = csub(e3, t3);
+}
+
+// Inverse 16-point DFT in place (two 8-point DFTs of the even / odd inputs, then the W16^m butterflies).
+LOFAR_HD void idft16(float2 *x)
+{
+    float2 e[8], o[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { e[i] = x[2 * i]; o[i] = x[2 * i + 1]; }
+    idft8(e);
+    idft8(o);
+    const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f, h = 0.70710678118654752440f;
+    const float wc[8] = {1.f, c1, h, s1, 0.f, -s1, -h, -c1};
+    const float ws[8] = {0.f, s1, h, c1, 1.f, c1, h, s1};
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        const float2 t = m == 0 ? o[0] : (m == 4 ? cmuli(o[4]) : cmul(o[m], make_float2(wc[m], ws[m])));
+        x[m] = cadd(e[m], t);
+        x[m + 8] = csub(e[m], t);
+    }
 }
 
 // Stockham pass with sub-transform length Ns (1, 8, 64): butterfly j (0..63) reads elements

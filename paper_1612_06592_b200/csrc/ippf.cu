@@ -8,7 +8,7 @@
 //   pre-pass : reads the K selected sub-band rows of Z for 16 slices (one 128-byte line per row),
 //              applies the trial phasor if asked, builds the packed half-spectrum V (fft_math.cuh)
 //              and stores it transposed -- slice-major -- into shared memory;
-//   FFT      : warp w transforms slice w with three Stockham radix-8 passes in place;
+//   FFT      : warp w transforms slice w in place: a radix-16 and a radix-32 pass (fft512_warp);
 //   FIR      : thread n owns output residues r = 2n, 2n+1; the 31-slice window (15 carried + 16 new)
 //              is read from the previous and current slice buffers, the 16 taps from shared memory;
 //              16 x 1024 contiguous output samples are written per step.
@@ -22,7 +22,7 @@ namespace lofar {
 namespace {
 
 constexpr int kThreads = 512;
-constexpr int kTwCount = 256 + 56 + 448;   // w1024[256], T2[7][8], T3[7][64]
+constexpr int kTwCount = 256 + 512;        // w1024[256], TB[32][16] = exp(2 pi i j r / 512)
 constexpr size_t kSmemBytes = (size_t)(2 * kStep * kRow + kP * kH + kTwCount) * sizeof(float2) + 256;
 
 struct Ctx {
@@ -133,38 +133,53 @@ __device__ __forceinline__ void prepass(const Ctx &c, const StepRegs &r, float2 
     }
 }
 
-// 512-point inverse complex FFT of one slice row by one warp, in place.
+// 512-point inverse complex FFT of one slice row by one warp, in place: 512 = 16 x 32.
+//   pass A: lane j does the 16-point DFT of elements j + 32 r and writes them to 16 j + m;
+//   pass B: butterfly j (0..15) is a 32-point DFT of elements j + 16 r with twiddles exp(2 pi i j r / 512);
+//           lanes j and j + 16 share it: each does the 16-point DFT of the even / odd r, the odd lane applies
+//           W32^m, the halves are exchanged with shuffles; outputs go to j + 16 m (m < 16 low lane, m >= 16 high).
 __device__ __forceinline__ void fft512_warp(float2 *row, const float2 *stw, int lane)
 {
+    float2 x[16];
 #pragma unroll
-    for (int pass = 0; pass < 3; ++pass) {
-        const int Ns = pass == 0 ? 1 : (pass == 1 ? 8 : 64);
-        float2 x[2][8];
+    for (int r = 0; r < 16; ++r) x[r] = row[pad(lane + 32 * r)];
+    idft16(x);
+    __syncwarp();
 #pragma unroll
-        for (int bf = 0; bf < 2; ++bf) {
-            const int j = lane + 32 * bf;
+    for (int m = 0; m < 16; ++m) row[pad(16 * lane + m)] = x[m];
+    __syncwarp();
+    const float2 *T = stw + 256 + lane;          // T[32 r' + lane] = exp(2 pi i j (hh + 2 r') / 512)
 #pragma unroll
-            for (int r = 0; r < 8; ++r) x[bf][r] = row[pad(stockham_src(j, r))];
-            if (pass == 1) {
-                const float2 *T = stw + 256 + (j & 7);
+    for (int r = 0; r < 16; ++r) x[r] = cmul(row[pad(lane + 32 * r)], T[32 * r]);
+    idft16(x);
+    const bool hi = lane >= 16;
+    if (hi) {
+        // W32^m = exp(2 pi i m / 32), m = 0..15
+        const float c[16] = {1.f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                             0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                             0.19509032201612826785f, 0.f, -0.19509032201612826785f, -0.38268343236508977173f,
+                             -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
+                             -0.92387953251128675613f, -0.98078528040323044913f};
+        const float sn[16] = {0.f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
+                              0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                              0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
+                              0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
+                              0.38268343236508977173f, 0.19509032201612826785f};
 #pragma unroll
-                for (int r = 1; r < 8; ++r) x[bf][r] = cmul(x[bf][r], T[(r - 1) * 8]);
-            } else if (pass == 2) {
-                const float2 *T = stw + 312 + (j & 63);
-#pragma unroll
-                for (int r = 1; r < 8; ++r) x[bf][r] = cmul(x[bf][r], T[(r - 1) * 64]);
-            }
-            idft8(x[bf]);
-        }
-        __syncwarp();
-#pragma unroll
-        for (int bf = 0; bf < 2; ++bf) {
-            const int j = lane + 32 * bf;
-#pragma unroll
-            for (int m = 0; m < 8; ++m) row[pad(stockham_dst(j, m, Ns))] = x[bf][m];
-        }
-        __syncwarp();
+        for (int m = 1; m < 16; ++m) x[m] = cmul(x[m], make_float2(c[m], sn[m]));
     }
+#pragma unroll
+    for (int m = 0; m < 16; ++m) {
+        float2 other;
+        other.x = __shfl_xor_sync(0xffffffffu, x[m].x, 16);
+        other.y = __shfl_xor_sync(0xffffffffu, x[m].y, 16);
+        x[m] = hi ? csub(other, x[m]) : cadd(x[m], other);     // low lane: E + O', high lane: E - O'
+    }
+    __syncwarp();
+    const int base = (lane & 15) + (hi ? 256 : 0);
+#pragma unroll
+    for (int m = 0; m < 16; ++m) row[pad(base + 16 * m)] = x[m];
+    __syncwarp();
 }
 
 __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
