@@ -275,14 +275,14 @@ def run_gpu(args):
     dom = max(kernels, key=lambda k: k["ms_per_step"])
     chain_bytes = w.input_bytes + w.nseries * w.T * w.M * 4
     # dram__bytes_read.sum + dram__bytes_write.sum over algorithmic bytes of the same launch, from the committed
-    # ncu --set full capture of configs[2] (profiles/r1_d_ncu_full.md); other workloads have no capture yet
-    ncu_ratio = {"ippf_kernel": 8.648592 / 8.650752, "beamform_tc_kernel": 6.287481 / 6.332375}
+    # ncu --set full capture of configs[2] (profiles/r1_f_ncu_full.md); other workloads have no capture yet
+    ncu_ratio = {"ippf_kernel": 8.694637 / 8.650752, "beamform_tc_kernel": 6.285303 / 6.332375}
     traffic = None
     if w.index == 2 and args.slices is None and dom["kernel"] in ncu_ratio:
         traffic = dom["algorithmic_GB_per_launch"] * ncu_ratio[dom["kernel"]]
     roofline = {"kernel": dom["kernel"], "bound": "hbm", "achieved": dom["achieved_GBps"], "peak": peak,
                 "unit": "GB/s", "frac": dom["achieved_GBps"] / peak, "traffic": traffic,
-                "traffic_unit": "GB per launch (ncu dram bytes, profiles/r1_d_ncu_full.md)",
+                "traffic_unit": "GB per launch (ncu dram bytes, profiles/r1_f_ncu_full.md)",
                 "algorithmic_GB_per_launch": dom["algorithmic_GB_per_launch"],
                 "ms_per_launch": dom["ms_per_launch"], "peak_source": peak_src,
                 "note": "achieved = algorithmic bytes per launch / mean launch duration, CUDA events on the "
