@@ -48,12 +48,13 @@ typedef struct lofar_plan lofar_plan; /* opaque, owned by the library */
 typedef enum {
     LOFAR_OK = 0,
     LOFAR_E_INVALID = 1,  /* NULL pointer, non-positive size, unsupported parameter value      */
-    LOFAR_E_SHAPE = 2,    /* sub-band range outside 0..M/2-1, slices > capacity, ...           */
+    LOFAR_E_SHAPE = 2,    /* sub-band range outside 0..M/2-1, state blob of another plan shape  */
     LOFAR_E_ALIGN = 3,    /* X base or row pitch not 16-byte aligned                           */
     LOFAR_E_ALLOC = 4,    /* host or device allocation failed                                  */
     LOFAR_E_CUDA = 5,     /* a CUDA runtime call failed (sticky error left for the caller)     */
     LOFAR_E_OVERFLOW = 6, /* more candidates than max_candidates (reported by lofar_stream_sync) */
-    LOFAR_E_STATE = 7     /* call not legal in the plan's current state                        */
+    LOFAR_E_STATE = 7     /* call not legal in the plan's current state, e.g. slices > the
+                             max_slices fixed by lofar_plan_set_input          */
 } lofar_status;
 
 typedef enum { LOFAR_CI8 = 0, LOFAR_CI16 = 1 } lofar_dtype;
@@ -93,14 +94,34 @@ LOFAR_API lofar_status lofar_plan_set_trials(lofar_plan *plan, int ntrials,
 /* h_host[16*1024] analysis prototype (sum = 1); NULL restores the default Kaiser design.
  * The synthesis taps are g = 1024*h (matched synthesis). */
 LOFAR_API lofar_status lofar_plan_set_filter(lofar_plan *plan, const double *h_host);
-/* Input sample type and the largest `slices` any later call will pass. */
+/* Input sample type and the largest `slices` any later call will pass (a larger value returns
+ * LOFAR_E_STATE from the compute calls). */
 LOFAR_API lofar_status lofar_plan_set_input(lofar_plan *plan, lofar_dtype dtype, int max_slices);
 /* Threshold kappa (candidate iff e/sigma > kappa, strict), envelope window W >= 1 samples
  * (e[n] = sqrt(mean of xhat[n-W+1..n]^2), reading A13), candidate buffer capacity. */
 LOFAR_API lofar_status lofar_plan_set_trigger(lofar_plan *plan, double kappa, int env_window,
                                               uint32_t max_candidates);
-/* Device bytes the plan holds or will hold (tables + history + scratch + staging). */
+/* Device bytes the plan allocates for the current settings: tables (weights, tensor-core operand
+ * images, trial phasors, taps, twiddles), 2 x carried history, envelope tail, beam-sum scratch,
+ * trigger partials, and the two streaming staging slots (input block, candidates, count, sigma)
+ * that lofar_stream_push adds on first use. */
 LOFAR_API lofar_status lofar_plan_workspace_bytes(lofar_plan *plan, size_t *bytes);
+/* Device-memory hooks (BASELINE.json:north_star "PyTorch used only for device
+ * memory"): every plan-owned DEVICE buffer is obtained with alloc(bytes, ctx) (NULL = failure ->
+ * LOFAR_E_ALLOC; at least 256-byte aligned) and returned with free_(ptr, ctx); both NULL restores
+ * cudaMalloc/cudaFree.  Buffers already held are released first with the allocator that made
+ * them (the plan's own streams are drained; work on caller streams must have completed).  The
+ * only memory the plan takes elsewhere is 256 bytes of pinned HOST memory for streaming counts. */
+LOFAR_API lofar_status lofar_plan_set_allocator(lofar_plan *plan, void *(*alloc)(size_t, void *),
+                                                void (*free_)(void *, void *), void *ctx);
+/* Upper bound in bytes for the beam-sum scratch of one time chunk (default 4 GiB).  A block longer
+ * than the chunk is processed chunk by chunk, history handed over on the device. */
+LOFAR_API lofar_status lofar_plan_set_scratch_limit(lofar_plan *plan, size_t bytes);
+/* How lofar_run_block would cut a block of `slices`: slices per scratch chunk, and the number and
+ * length (slices) of the independent time spans one inverse-PPF launch is divided into.  Host only;
+ * lets tests aim parity windows at chunk and span boundaries. */
+LOFAR_API lofar_status lofar_plan_chunking(lofar_plan *plan, int slices, int64_t *chunk_slices,
+                                           int *spans, int *span_slices);
 
 /* ---- stage calls (all pointers device) ------------------------------------------------------
  * X: [S][2][K][slices][re,im] int8 or int16, little endian, time fastest; base and row pitch
@@ -131,8 +152,8 @@ LOFAR_API lofar_status lofar_run_block(lofar_plan *plan, const void *X, int slic
                                        void *stream);
 
 /* ---- streaming driver (a6; BASELINE.json:configs[4]) -------------------------------------------
- * lofar_stream_reset: waits for the plan's own streams, zeroes the carried history and the
- * stream offset.
+ * lofar_stream_reset: waits for the plan's own streams and resets the stream offset; the carried
+ * history is zeroed on the stream of the next compute call (no device-wide synchronisation).
  * lofar_stream_push: X_host is a HOST buffer (pinned for copy/compute overlap; pageable works
  * but serialises) laid out as X above.  The block is copied into one of two plan-owned device
  * buffers on a copy stream while the previous block computes on a compute stream; then
@@ -147,6 +168,15 @@ LOFAR_API lofar_status lofar_stream_push(lofar_plan *plan, const void *X_host, i
                                          float *series, lofar_candidate *cand_host,
                                          uint32_t *count_host, float *sigma_host);
 LOFAR_API lofar_status lofar_stream_sync(lofar_plan *plan);
+/* Checkpoint / resume of the carried state: a small header (stream offset,
+ * shape), the 15-slice synthesis history [B*D][15][1024] fp32 and the env_window-1 envelope tail.
+ * HOST buffers of lofar_stream_state_bytes bytes.  Both calls block: they drain the plan's own
+ * streams and copy synchronously (work the caller enqueued on its own streams must have
+ * completed).  set_state on a plan of another shape returns LOFAR_E_SHAPE; before
+ * lofar_plan_set_input has fixed the capacity both return LOFAR_E_STATE. */
+LOFAR_API lofar_status lofar_stream_state_bytes(lofar_plan *plan, size_t *bytes);
+LOFAR_API lofar_status lofar_stream_get_state(lofar_plan *plan, void *state_host, size_t bytes);
+LOFAR_API lofar_status lofar_stream_set_state(lofar_plan *plan, const void *state_host, size_t bytes);
 
 /* Per-kernel device timing (measurement aid, PAPER-independent).  With profiling enabled every kernel
  * the plan launches is bracketed by CUDA events on its own stream.  lofar_plan_profile_read waits for

@@ -26,7 +26,9 @@ assert CANDIDATE_DTYPE.itemsize == 24
 EXPORTS = (
     "lofar_plan_create", "lofar_plan_destroy", "lofar_plan_set_band", "lofar_plan_set_delays",
     "lofar_plan_set_trials", "lofar_plan_set_filter", "lofar_plan_set_input",
-    "lofar_plan_set_trigger", "lofar_plan_workspace_bytes", "lofar_beamform_dedisperse",
+    "lofar_plan_set_trigger", "lofar_plan_workspace_bytes", "lofar_plan_set_allocator",
+    "lofar_plan_set_scratch_limit", "lofar_plan_chunking", "lofar_stream_state_bytes",
+    "lofar_stream_get_state", "lofar_stream_set_state", "lofar_beamform_dedisperse",
     "lofar_inverse_ppf", "lofar_trigger", "lofar_run_block", "lofar_stream_reset",
     "lofar_stream_push", "lofar_stream_sync", "lofar_plan_profile", "lofar_plan_profile_read",
     "lofar_plan_launch_count", "lofar_status_string",
@@ -63,6 +65,12 @@ def load() -> ctypes.CDLL:
         "lofar_plan_set_input": (i, [vp, i, i]),
         "lofar_plan_set_trigger": (i, [vp, d, i, u32]),
         "lofar_plan_workspace_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
+        "lofar_plan_set_allocator": (i, [vp, vp, vp, vp]),
+        "lofar_plan_set_scratch_limit": (i, [vp, c.c_size_t]),
+        "lofar_plan_chunking": (i, [vp, i, c.POINTER(c.c_int64), c.POINTER(i), c.POINTER(i)]),
+        "lofar_stream_state_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
+        "lofar_stream_get_state": (i, [vp, vp, c.c_size_t]),
+        "lofar_stream_set_state": (i, [vp, vp, c.c_size_t]),
         "lofar_beamform_dedisperse": (i, [vp, vp, i, vp, vp]),
         "lofar_inverse_ppf": (i, [vp, vp, i, vp, vp]),
         "lofar_trigger": (i, [vp, vp, i, vp, vp, vp, vp]),
@@ -128,6 +136,7 @@ class Plan:
         if getattr(self, "_h", None):
             self._lib.lofar_plan_destroy(self._h)
             self._h = None
+            self._alloc_thunks = None
 
     def __del__(self):
         try:
@@ -172,6 +181,48 @@ class Plan:
         n = ctypes.c_size_t()
         _check(self._lib.lofar_plan_workspace_bytes(self._h, ctypes.byref(n)), "lofar_plan_workspace_bytes")
         return int(n.value)
+
+    ALLOC_FN = ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+    FREE_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
+
+    def set_allocator(self, alloc=None, free=None):
+        """alloc(nbytes) -> device address (0 on failure), free(address); None/None restores cudaMalloc.
+        The ctypes thunks are kept alive on the Plan for as long as the library may call them."""
+        if alloc is None and free is None:
+            _check(self._lib.lofar_plan_set_allocator(self._h, None, None, None), "lofar_plan_set_allocator")
+            self._alloc_thunks = None
+            return
+        a = self.ALLOC_FN(lambda n, ctx: alloc(n) or None)
+        f = self.FREE_FN(lambda ptr, ctx: free(ptr))
+        _check(self._lib.lofar_plan_set_allocator(self._h, ctypes.cast(a, ctypes.c_void_p),
+                                                  ctypes.cast(f, ctypes.c_void_p), None), "lofar_plan_set_allocator")
+        self._alloc_thunks = (a, f)
+
+    def set_torch_allocator(self):
+        """Plan memory from torch's caching allocator (north_star: "PyTorch used only for device memory")."""
+        import torch
+        self.set_allocator(torch.cuda.caching_allocator_alloc, torch.cuda.caching_allocator_delete)
+
+    def set_scratch_limit(self, nbytes: int):
+        _check(self._lib.lofar_plan_set_scratch_limit(self._h, int(nbytes)), "lofar_plan_set_scratch_limit")
+
+    def chunking(self, slices: int):
+        """(slices per scratch chunk, spans per inverse-PPF launch, slices per span)."""
+        zc, ns, sl = ctypes.c_int64(), ctypes.c_int(), ctypes.c_int()
+        _check(self._lib.lofar_plan_chunking(self._h, slices, ctypes.byref(zc), ctypes.byref(ns), ctypes.byref(sl)),
+               "lofar_plan_chunking")
+        return int(zc.value), int(ns.value), int(sl.value)
+
+    def get_state(self) -> np.ndarray:
+        n = ctypes.c_size_t()
+        _check(self._lib.lofar_stream_state_bytes(self._h, ctypes.byref(n)), "lofar_stream_state_bytes")
+        buf = np.zeros(n.value, dtype=np.uint8)
+        _check(self._lib.lofar_stream_get_state(self._h, buf.ctypes.data, buf.size), "lofar_stream_get_state")
+        return buf
+
+    def set_state(self, buf: np.ndarray, allow=()):
+        buf = np.ascontiguousarray(buf, dtype=np.uint8)
+        return _check(self._lib.lofar_stream_set_state(self._h, buf.ctypes.data, buf.size), "lofar_stream_set_state", allow)
 
     def launch_count(self) -> int:
         return int(self._lib.lofar_plan_launch_count(self._h))

@@ -14,7 +14,6 @@ namespace {
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr double kDispersion = 1.343e9;   // phi(f) = 2 pi * 1.343e9 * STEC / f  (BASELINE.json:configs[0])
 constexpr int kMfft = 1024, kTaps = 16, kHalf = 512, kStepSlices = 16;
-constexpr size_t kScratchBudget = (size_t)4 << 30;   // bytes of beam-sum scratch per time chunk
 constexpr int kCountRing = 64;
 
 #define CU(call)                                   \
@@ -28,29 +27,55 @@ lofar_status dev_alloc(lofar_plan *p, T **ptr, size_t count)
     *ptr = nullptr;
     if (count == 0) return LOFAR_OK;
     void *v = nullptr;
-    cudaError_t e = cudaMalloc(&v, count * sizeof(T));
-    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return LOFAR_E_ALLOC; }
-    if (e != cudaSuccess) return LOFAR_E_CUDA;
+    if (p->alloc_fn) {
+        v = p->alloc_fn(count * sizeof(T), p->alloc_ctx);
+        if (!v) return LOFAR_E_ALLOC;
+    } else {
+        cudaError_t e = cudaMalloc(&v, count * sizeof(T));
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return LOFAR_E_ALLOC; }
+        if (e != cudaSuccess) return LOFAR_E_CUDA;
+    }
     *ptr = static_cast<T *>(v);
     p->device_bytes += count * sizeof(T);
     return LOFAR_OK;
 }
 
 template <typename T>
-void dev_free(T *&ptr)
+void dev_free(lofar_plan *p, T *&ptr)
 {
-    if (ptr) cudaFree(ptr);
+    if (ptr) {
+        if (p->free_fn) p->free_fn(const_cast<void *>(static_cast<const void *>(ptr)), p->alloc_ctx);
+        else cudaFree(const_cast<void *>(static_cast<const void *>(ptr)));
+    }
     ptr = nullptr;
+}
+
+void free_staging(lofar_plan *p)
+{
+    for (int i = 0; i < 2; ++i) {
+        char *x = static_cast<char *>(p->dX[i]);
+        dev_free(p, x);
+        p->dX[i] = nullptr;
+        dev_free(p, p->dCand[i]); dev_free(p, p->dCount[i]); dev_free(p, p->dSigma[i]);
+    }
+    p->dX_bytes = 0;
+}
+
+// Waits for the plan's own streams; buffers may then be released (caller streams are the caller's to order).
+void quiesce(lofar_plan *p)
+{
+    if (p->s_copy) cudaStreamSynchronize(p->s_copy);
+    if (p->s_comp) cudaStreamSynchronize(p->s_comp);
 }
 
 void free_tables(lofar_plan *p)
 {
-    dev_free(p->dWimg);
-    dev_free(p->dW); dev_free(p->dDph); dev_free(p->dGs); dev_free(p->dTw);
-    dev_free(p->dHist[0]); dev_free(p->dHist[1]); dev_free(p->dTail);
-    dev_free(p->dZ); dev_free(p->dPartial); dev_free(p->dChunkMax);
-    for (int i = 0; i < 2; ++i) { dev_free(p->dX[i]); dev_free(p->dCand[i]); dev_free(p->dCount[i]); dev_free(p->dSigma[i]); }
-    p->dX_bytes = 0;
+    quiesce(p);
+    dev_free(p, p->dWimg);
+    dev_free(p, p->dW); dev_free(p, p->dDph); dev_free(p, p->dGs); dev_free(p, p->dTw);
+    dev_free(p, p->dHist[0]); dev_free(p, p->dHist[1]); dev_free(p, p->dTail);
+    dev_free(p, p->dZ); dev_free(p, p->dPartial); dev_free(p, p->dChunkMax);
+    free_staging(p);
     p->device_bytes = 0;
     p->built = false;
 }
@@ -105,6 +130,47 @@ long long round_up(long long v, long long m) { return (v + m - 1) / m * m; }
 
 size_t sample_bytes(const lofar_plan *p) { return p->dtype == LOFAR_CI16 ? 4 : 2; }
 
+// Element counts of every plan-owned device buffer for the current settings: build() allocates exactly
+// these, lofar_plan_workspace_bytes reports their sum.
+struct Layout {
+    bool tc;                 // tensor-core operand images wanted (int8 input)
+    size_t W, Dph, gs, tw, wimg, hist, tail, Z, partial, chunkmax;
+    size_t x_bytes, cand, sigma;   // streaming staging (per slot)
+    long long cap, zchunk, nsteps;
+    size_t table_bytes() const
+    {
+        return (W + Dph + gs + tw + Z) * sizeof(float2) + wimg * sizeof(unsigned short) +
+               (2 * hist + tail + chunkmax) * sizeof(float) + partial * sizeof(double);
+    }
+    size_t staging_bytes() const
+    {
+        return 2 * (x_bytes + cand * sizeof(lofar_candidate) + sizeof(uint32_t) + sigma * sizeof(float));
+    }
+};
+
+Layout layout(const lofar_plan *p)
+{
+    Layout L{};
+    const size_t S = p->S, K = p->K, B = p->B, D = p->D, ns = B * D;
+    L.tc = p->dtype == LOFAR_CI8 && p->S <= 32 && p->B <= 128;
+    L.W = K * B * S; L.Dph = D * K; L.gs = (size_t)kTaps * kHalf; L.tw = 256 + 512;
+    L.wimg = L.tc ? K * 2 * tc_image_halfs(p->S, p->B) : 0;
+    L.hist = ns * (kTaps - 1) * kMfft;
+    L.tail = ns * (size_t)(p->env_window - 1);
+    L.cap = round_up(p->max_slices > 0 ? p->max_slices : kStepSlices, kStepSlices);
+    long long zc = (long long)(p->scratch_limit / (B * K * sizeof(float2)));
+    zc = zc >= 1024 ? zc / 1024 * 1024 : zc / 32 * 32;
+    if (zc < 32) zc = 32;
+    L.zchunk = round_up(zc < L.cap ? zc : L.cap, 32);      // whole 32-slice tiles of the scratch layout
+    L.Z = B * K * (size_t)L.zchunk;
+    L.nsteps = L.cap / kStepSlices;
+    L.partial = ns * (size_t)L.nsteps;
+    L.chunkmax = ns * (size_t)L.nsteps;
+    L.x_bytes = S * 2 * K * (size_t)(p->max_slices > 0 ? p->max_slices : 0) * sample_bytes(p);
+    L.cand = p->max_cand; L.sigma = ns;
+    return L;
+}
+
 lofar_status build(lofar_plan *p)
 {
     free_tables(p);
@@ -112,13 +178,15 @@ lofar_status build(lofar_plan *p)
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev));
     if (ippf_configure() != 0) return LOFAR_E_CUDA;
-    const int S = p->S, K = p->K, B = p->B, D = p->D, ns = B * D;
+    const Layout L = layout(p);
+    if (L.tc && tc_configure() != 0) return LOFAR_E_CUDA;
+    const int S = p->S, K = p->K, B = p->B, D = p->D;
 
     // ---- tables, in double on the host, rounded once to fp32 ----
-    std::vector<float2> W((size_t)K * B * S), Dph((size_t)D * K), gs((size_t)kTaps * kHalf), tw(256 + 512);
-    const bool tc = p->dtype == LOFAR_CI8 && S <= 32 && B <= 128;
+    std::vector<float2> W(L.W), Dph(L.Dph), gs(L.gs), tw(L.tw);
+    const bool tc = L.tc;
     const size_t img = tc ? tc_image_halfs(S, B) : 0;
-    std::vector<unsigned short> wimg((size_t)K * 2 * img);
+    std::vector<unsigned short> wimg(L.wimg);
     std::vector<double> wre((size_t)B * S), wim((size_t)B * S);
     for (int j = 0; j < K; ++j) {
         const double f = p->f_zone + (double)(p->k0 + j) * (p->clock / kMfft);
@@ -144,12 +212,12 @@ lofar_status build(lofar_plan *p)
         for (int jj = 0; jj < 16; ++jj) tw[256 + r * 16 + jj] = unit_phasor((double)(jj * r) / 512.0);
 
     lofar_status st;
-    if ((st = dev_alloc(p, &p->dW, W.size())) != LOFAR_OK) return st;
-    if ((st = dev_alloc(p, &p->dDph, Dph.size())) != LOFAR_OK) return st;
-    if ((st = dev_alloc(p, &p->dGs, gs.size())) != LOFAR_OK) return st;
-    if ((st = dev_alloc(p, &p->dTw, tw.size())) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dW, L.W)) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dDph, L.Dph)) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dGs, L.gs)) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dTw, L.tw)) != LOFAR_OK) return st;
     if (tc) {
-        if ((st = dev_alloc(p, &p->dWimg, wimg.size())) != LOFAR_OK) return st;
+        if ((st = dev_alloc(p, &p->dWimg, L.wimg)) != LOFAR_OK) return st;
         CU(cudaMemcpy(p->dWimg, wimg.data(), wimg.size() * sizeof(unsigned short), cudaMemcpyHostToDevice));
     }
     CU(cudaMemcpy(p->dW, W.data(), W.size() * sizeof(float2), cudaMemcpyHostToDevice));
@@ -158,31 +226,39 @@ lofar_status build(lofar_plan *p)
     CU(cudaMemcpy(p->dTw, tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice));
 
     // ---- carried state ----
-    const size_t hist = (size_t)ns * (kTaps - 1) * kMfft;
     for (int i = 0; i < 2; ++i) {
-        if ((st = dev_alloc(p, &p->dHist[i], hist)) != LOFAR_OK) return st;
-        CU(cudaMemset(p->dHist[i], 0, hist * sizeof(float)));
+        if ((st = dev_alloc(p, &p->dHist[i], L.hist)) != LOFAR_OK) return st;
+        CU(cudaMemset(p->dHist[i], 0, L.hist * sizeof(float)));
     }
     p->hist_parity = 0;
-    if (p->env_window > 1) {
-        if ((st = dev_alloc(p, &p->dTail, (size_t)ns * (p->env_window - 1))) != LOFAR_OK) return st;
-        CU(cudaMemset(p->dTail, 0, (size_t)ns * (p->env_window - 1) * sizeof(float)));
+    if (L.tail) {
+        if ((st = dev_alloc(p, &p->dTail, L.tail)) != LOFAR_OK) return st;
+        CU(cudaMemset(p->dTail, 0, L.tail * sizeof(float)));
     }
     p->offset = 0;
+    p->reset_pending = false;
 
     // ---- scratch sized for max_slices ----
-    const long long cap = round_up(p->max_slices > 0 ? p->max_slices : kStepSlices, kStepSlices);
-    long long zc = (long long)(kScratchBudget / ((size_t)B * K * sizeof(float2)));
-    zc = zc / 1024 * 1024;
-    if (zc < 1024) zc = 1024;
-    p->zchunk = round_up(zc < cap ? zc : cap, 32);      // whole 32-slice tiles of the scratch layout
-    if ((st = dev_alloc(p, &p->dZ, (size_t)B * K * p->zchunk)) != LOFAR_OK) return st;
-    const long long nsteps = cap / kStepSlices;
-    p->partial_pitch = (int)nsteps;
-    p->chunkmax_pitch = nsteps;
-    if ((st = dev_alloc(p, &p->dPartial, (size_t)ns * nsteps)) != LOFAR_OK) return st;
-    if ((st = dev_alloc(p, &p->dChunkMax, (size_t)ns * nsteps)) != LOFAR_OK) return st;
+    p->zchunk = L.zchunk;
+    if ((st = dev_alloc(p, &p->dZ, L.Z)) != LOFAR_OK) return st;
+    CU(cudaMemset(p->dZ, 0, L.Z * sizeof(float2)));
+    p->partial_pitch = (int)L.nsteps;
+    p->chunkmax_pitch = L.nsteps;
+    if ((st = dev_alloc(p, &p->dPartial, L.partial)) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dChunkMax, L.chunkmax)) != LOFAR_OK) return st;
     p->built = true;
+    return LOFAR_OK;
+}
+
+// Zeroes the carried state on the stream of the compute call that follows a lofar_stream_reset.
+lofar_status apply_reset(lofar_plan *p, cudaStream_t st)
+{
+    if (!p->reset_pending) return LOFAR_OK;
+    const size_t hist = (size_t)p->B * p->D * (kTaps - 1) * kMfft * sizeof(float);
+    CU(cudaMemsetAsync(p->dHist[0], 0, hist, st));
+    CU(cudaMemsetAsync(p->dHist[1], 0, hist, st));
+    if (p->dTail) CU(cudaMemsetAsync(p->dTail, 0, (size_t)p->B * p->D * (p->env_window - 1) * sizeof(float), st));
+    p->reset_pending = false;
     return LOFAR_OK;
 }
 
@@ -191,8 +267,11 @@ lofar_status ensure(lofar_plan *p, int slices)
     if (!p) return LOFAR_E_INVALID;
     if (slices <= 0) return LOFAR_E_INVALID;
     if (p->max_slices <= 0) { p->max_slices = slices; p->built = false; }
-    if (slices > p->max_slices) return LOFAR_E_SHAPE;
-    if (!p->built) return build(p);
+    if (slices > p->max_slices) return LOFAR_E_STATE;   // capacity fixed by lofar_plan_set_input
+    if (!p->built) {
+        const lofar_status st = build(p);
+        if (st != LOFAR_OK) { free_tables(p); return st; }
+    }
     return LOFAR_OK;
 }
 
@@ -336,8 +415,9 @@ lofar_status lofar_plan_create(lofar_plan **out, int stations, int subbands, int
 void lofar_plan_destroy(lofar_plan *p)
 {
     if (!p) return;
-    if (p->s_copy) { cudaStreamSynchronize(p->s_copy); cudaStreamDestroy(p->s_copy); }
-    if (p->s_comp) { cudaStreamSynchronize(p->s_comp); cudaStreamDestroy(p->s_comp); }
+    free_tables(p);                    // drains the plan's own streams first
+    if (p->s_copy) { cudaStreamDestroy(p->s_copy); p->s_copy = nullptr; }
+    if (p->s_comp) { cudaStreamDestroy(p->s_comp); p->s_comp = nullptr; }
     for (int i = 0; i < 2; ++i) {
         if (p->ev_copied[i]) cudaEventDestroy(p->ev_copied[i]);
         if (p->ev_done[i]) cudaEventDestroy(p->ev_done[i]);
@@ -345,7 +425,6 @@ void lofar_plan_destroy(lofar_plan *p)
     if (p->hCount) cudaFreeHost(p->hCount);
     for (auto &r : p->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto e : p->prof_pool) cudaEventDestroy(e);
-    free_tables(p);
     delete p;
 }
 
@@ -406,20 +485,45 @@ lofar_status lofar_plan_set_trigger(lofar_plan *p, double kappa, int env_window,
 lofar_status lofar_plan_workspace_bytes(lofar_plan *p, size_t *bytes)
 {
     if (!p || !bytes) return LOFAR_E_INVALID;
-    if (p->built) { *bytes = p->device_bytes; return LOFAR_OK; }
-    // what build() will allocate for the current settings (streaming buffers excluded until used)
-    const size_t ns = (size_t)p->B * p->D;
-    const long long cap = round_up(p->max_slices > 0 ? p->max_slices : kStepSlices, kStepSlices);
-    long long zc = (long long)(kScratchBudget / ((size_t)p->B * p->K * sizeof(float2))) / 1024 * 1024;
-    if (zc < 1024) zc = 1024;
-    if (zc > cap) zc = round_up(cap, 32);
-    size_t b = 0;
-    b += ((size_t)p->K * p->B * p->S + (size_t)p->D * p->K + (size_t)kTaps * kHalf + 768) * sizeof(float2);
-    b += 2 * ns * (kTaps - 1) * kMfft * sizeof(float);
-    b += ns * (size_t)(p->env_window - 1) * sizeof(float);
-    b += (size_t)p->B * p->K * zc * sizeof(float2);
-    b += ns * (size_t)(cap / kStepSlices) * (sizeof(double) + sizeof(float));
-    *bytes = b;
+    const Layout L = layout(p);
+    *bytes = L.table_bytes() + L.staging_bytes();
+    return LOFAR_OK;
+}
+
+lofar_status lofar_plan_set_allocator(lofar_plan *p, void *(*alloc)(size_t, void *), void (*free_)(void *, void *),
+                                      void *ctx)
+{
+    if (!p || ((alloc == nullptr) != (free_ == nullptr))) return LOFAR_E_INVALID;
+    free_tables(p);                    // with the allocator that made them
+    p->alloc_fn = alloc; p->free_fn = free_; p->alloc_ctx = ctx;
+    return LOFAR_OK;
+}
+
+lofar_status lofar_plan_set_scratch_limit(lofar_plan *p, size_t bytes)
+{
+    if (!p || bytes == 0) return LOFAR_E_INVALID;
+    p->scratch_limit = bytes;
+    p->built = false;
+    return LOFAR_OK;
+}
+
+lofar_status lofar_plan_chunking(lofar_plan *p, int slices, int64_t *chunk_slices, int *spans, int *span_slices)
+{
+    if (!p || slices <= 0 || !chunk_slices || !spans || !span_slices) return LOFAR_E_INVALID;
+    if (p->max_slices > 0 && slices > p->max_slices) return LOFAR_E_STATE;
+    const int keep = p->max_slices;
+    if (p->max_slices <= 0) p->max_slices = slices;
+    const Layout L = layout(p);
+    p->max_slices = keep;
+    *chunk_slices = L.zchunk;
+    int sms = p->num_sms;
+    if (!p->built) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        else { cudaGetLastError(); sms = 148; }
+    }
+    const long long nc = slices < L.zchunk ? slices : L.zchunk;
+    plan_spans((nc + kStepSlices - 1) / kStepSlices, p->B * p->D, sms, spans, span_slices);
     return LOFAR_OK;
 }
 
@@ -447,6 +551,7 @@ lofar_status lofar_inverse_ppf(lofar_plan *p, const void *Z, int slices, float *
     if (s != LOFAR_OK) return s;
     if (!Z || !series) return LOFAR_E_INVALID;
     if (reinterpret_cast<size_t>(Z) & 7 || reinterpret_cast<size_t>(series) & 7) return LOFAR_E_ALIGN;
+    if ((s = apply_reset(p, static_cast<cudaStream_t>(stream))) != LOFAR_OK) return s;
     int partial0 = 0;
     return do_ippf(p, static_cast<const float2 *>(Z), slices, 0, slices, 0, series, (long long)slices * kMfft, 0,
                    &partial0, 0, static_cast<cudaStream_t>(stream));
@@ -459,6 +564,7 @@ lofar_status lofar_trigger(lofar_plan *p, const float *series, int slices, lofar
     if (s != LOFAR_OK) return s;
     if (!series || !cand || !count || !sigma) return LOFAR_E_INVALID;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if ((s = apply_reset(p, st)) != LOFAR_OK) return s;
     const long long N = (long long)slices * kMfft;
     TriggerArgs t = trigger_args(p, series, N, cand, count, sigma);
     t.nparts = (int)t.nchunks;
@@ -483,6 +589,7 @@ lofar_status lofar_run_block(lofar_plan *p, const void *X, int slices, float *se
     if (s != LOFAR_OK) return s;
     if (!series || !cand || !count || !sigma) return LOFAR_E_INVALID;
     if ((s = check_x(p, X, slices)) != LOFAR_OK) return s;
+    if ((s = apply_reset(p, static_cast<cudaStream_t>(stream))) != LOFAR_OK) return s;
     return run_block_impl(p, X, slices, series, cand, count, sigma, static_cast<cudaStream_t>(stream));
 }
 
@@ -494,14 +601,7 @@ lofar_status lofar_stream_reset(lofar_plan *p)
     p->offset = 0;
     p->pushes = 0;
     p->slot_used[0] = p->slot_used[1] = false;
-    if (p->built) {
-        CU(cudaDeviceSynchronize());
-        const size_t hist = (size_t)p->B * p->D * (kTaps - 1) * kMfft * sizeof(float);
-        CU(cudaMemset(p->dHist[0], 0, hist));
-        CU(cudaMemset(p->dHist[1], 0, hist));
-        if (p->dTail) CU(cudaMemset(p->dTail, 0, (size_t)p->B * p->D * (p->env_window - 1) * sizeof(float)));
-        CU(cudaDeviceSynchronize());
-    }
+    p->reset_pending = p->built;       // zeroing is enqueued on the stream of the next compute call
     return LOFAR_OK;
 }
 
@@ -524,16 +624,16 @@ lofar_status lofar_stream_push(lofar_plan *p, const void *X_host, int slices, fl
         CU(cudaMallocHost(reinterpret_cast<void **>(&p->hCount), kCountRing * sizeof(uint32_t)));
     }
     if (!p->dX[0]) {
-        const size_t bytes = (size_t)p->S * 2 * p->K * (size_t)p->max_slices * sample_bytes(p);
-        for (int i = 0; i < 2; ++i) {
+        const Layout L = layout(p);
+        for (int i = 0; i < 2 && s == LOFAR_OK; ++i) {
             char *x = nullptr;
-            if ((s = dev_alloc(p, &x, bytes)) != LOFAR_OK) return s;
-            p->dX[i] = x;
-            if ((s = dev_alloc(p, &p->dCand[i], (size_t)p->max_cand)) != LOFAR_OK) return s;
-            if ((s = dev_alloc(p, &p->dCount[i], 1)) != LOFAR_OK) return s;
-            if ((s = dev_alloc(p, &p->dSigma[i], (size_t)ns)) != LOFAR_OK) return s;
+            if ((s = dev_alloc(p, &x, L.x_bytes)) == LOFAR_OK) p->dX[i] = x;
+            if (s == LOFAR_OK) s = dev_alloc(p, &p->dCand[i], L.cand);
+            if (s == LOFAR_OK) s = dev_alloc(p, &p->dCount[i], 1);
+            if (s == LOFAR_OK) s = dev_alloc(p, &p->dSigma[i], L.sigma);
         }
-        p->dX_bytes = bytes;
+        if (s != LOFAR_OK) { free_staging(p); return s; }   // nothing half-allocated is left behind
+        p->dX_bytes = L.x_bytes;
     }
     const int slot = (int)(p->push_index & 1);
     const size_t bytes = (size_t)p->S * 2 * p->K * (size_t)slices * sample_bytes(p);
@@ -541,6 +641,7 @@ lofar_status lofar_stream_push(lofar_plan *p, const void *X_host, int slices, fl
     CU(cudaMemcpyAsync(p->dX[slot], X_host, bytes, cudaMemcpyHostToDevice, p->s_copy));
     CU(cudaEventRecord(p->ev_copied[slot], p->s_copy));
     CU(cudaStreamWaitEvent(p->s_comp, p->ev_copied[slot], 0));
+    if ((s = apply_reset(p, p->s_comp)) != LOFAR_OK) return s;
     s = run_block_impl(p, p->dX[slot], slices, series, p->dCand[slot], p->dCount[slot], p->dSigma[slot], p->s_comp);
     if (s != LOFAR_OK) return s;
     CU(cudaMemcpyAsync(&p->hCount[p->pushes], p->dCount[slot], sizeof(uint32_t), cudaMemcpyDeviceToHost, p->s_comp));
@@ -567,6 +668,73 @@ lofar_status lofar_stream_sync(lofar_plan *p)
     for (int i = 0; i < p->pushes; ++i) over = over || (p->hCount[i] > p->max_cand);
     p->pushes = 0;
     return over ? LOFAR_E_OVERFLOW : LOFAR_OK;
+}
+
+// ---- carried state for checkpoint / resume: header, history, envelope tail ----
+namespace {
+struct StateHeader { uint32_t magic, nseries, taps, fft, env_window, reserved; uint64_t offset; };
+constexpr uint32_t kStateMagic = 0x4c4f4631u;   // "LOF1"
+size_t state_bytes(const lofar_plan *p)
+{
+    const size_t ns = (size_t)p->B * p->D;
+    return sizeof(StateHeader) + ns * (kTaps - 1) * kMfft * sizeof(float) + ns * (size_t)(p->env_window - 1) * sizeof(float);
+}
+}  // namespace
+
+lofar_status lofar_stream_state_bytes(lofar_plan *p, size_t *bytes)
+{
+    if (!p || !bytes) return LOFAR_E_INVALID;
+    *bytes = state_bytes(p);
+    return LOFAR_OK;
+}
+
+lofar_status lofar_stream_get_state(lofar_plan *p, void *state_host, size_t bytes)
+{
+    if (!p || !state_host) return LOFAR_E_INVALID;
+    if (bytes < state_bytes(p)) return LOFAR_E_SHAPE;
+    if (!p->built) {
+        if (p->max_slices <= 0) return LOFAR_E_STATE;
+        const lofar_status st = build(p);
+        if (st != LOFAR_OK) { free_tables(p); return st; }
+    }
+    quiesce(p);
+    const size_t ns = (size_t)p->B * p->D, hist = ns * (kTaps - 1) * kMfft * sizeof(float);
+    const size_t tail = ns * (size_t)(p->env_window - 1) * sizeof(float);
+    StateHeader h{kStateMagic, (uint32_t)ns, (uint32_t)kTaps, (uint32_t)kMfft, (uint32_t)p->env_window, 0u, p->offset};
+    char *dst = static_cast<char *>(state_host);
+    std::memcpy(dst, &h, sizeof(h));
+    if (p->reset_pending) {
+        std::memset(dst + sizeof(h), 0, hist + tail);
+        return LOFAR_OK;
+    }
+    CU(cudaMemcpy(dst + sizeof(h), p->dHist[p->hist_parity], hist, cudaMemcpyDeviceToHost));
+    if (tail) CU(cudaMemcpy(dst + sizeof(h) + hist, p->dTail, tail, cudaMemcpyDeviceToHost));
+    return LOFAR_OK;
+}
+
+lofar_status lofar_stream_set_state(lofar_plan *p, const void *state_host, size_t bytes)
+{
+    if (!p || !state_host) return LOFAR_E_INVALID;
+    if (bytes < state_bytes(p)) return LOFAR_E_SHAPE;
+    StateHeader h;
+    std::memcpy(&h, state_host, sizeof(h));
+    const size_t ns = (size_t)p->B * p->D;
+    if (h.magic != kStateMagic || h.nseries != ns || h.taps != (uint32_t)kTaps || h.fft != (uint32_t)kMfft ||
+        h.env_window != (uint32_t)p->env_window)
+        return LOFAR_E_SHAPE;
+    if (!p->built) {
+        if (p->max_slices <= 0) return LOFAR_E_STATE;
+        const lofar_status st = build(p);
+        if (st != LOFAR_OK) { free_tables(p); return st; }
+    }
+    quiesce(p);
+    const size_t hist = ns * (kTaps - 1) * kMfft * sizeof(float), tail = ns * (size_t)(p->env_window - 1) * sizeof(float);
+    const char *src = static_cast<const char *>(state_host);
+    CU(cudaMemcpy(p->dHist[p->hist_parity], src + sizeof(h), hist, cudaMemcpyHostToDevice));
+    if (tail) CU(cudaMemcpy(p->dTail, src + sizeof(h) + hist, tail, cudaMemcpyHostToDevice));
+    p->offset = h.offset;
+    p->reset_pending = false;
+    return LOFAR_OK;
 }
 
 lofar_status lofar_plan_profile(lofar_plan *p, int enable)

@@ -249,6 +249,13 @@ bool tc_supported(const BeamformArgs &a)
            (a.t0 % 8) == 0;
 }
 
+// Per device (function attributes are per context): called from every plan build, result checked there.
+int tc_configure()
+{
+    cudaError_t e = cudaFuncSetAttribute(beamform_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    return e == cudaSuccess ? 0 : -1;
+}
+
 int launch_beamform_tc(const BeamformArgs &b, const void *wimg, cudaStream_t st)
 {
     if (b.nt <= 0) return 0;
@@ -263,11 +270,6 @@ int launch_beamform_tc(const BeamformArgs &b, const void *wimg, cudaStream_t st)
     a.tiles_per_cta = tiles < 32 ? (int)tiles : 32;
     dim3 grid((unsigned)((tiles + a.tiles_per_cta - 1) / a.tiles_per_cta), (unsigned)b.K);
     const size_t smem = (size_t)a.kchunks * kLboA + 2 * (size_t)a.img16 * 16 + 16;
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(beamform_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        configured = true;
-    }
     beamform_tc_kernel<<<grid, kTcThreads, smem, st>>>(a);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }

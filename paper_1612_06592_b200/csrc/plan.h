@@ -40,7 +40,7 @@ struct IppfArgs {
     const float *hist_in; // [nseries][15][1024]
     float *hist_out;
     const float2 *gs;     // [16][512] synthesis taps (g[2n + 1024 t], g[2n+1 + 1024 t])
-    const float2 *tw;     // twiddles: w1024[256], T2[7][8], T3[7][64]
+    const float2 *tw;     // twiddles: w1024[256] (pre-pass), TB[32][16] = exp(2 pi i j r / 512) (radix-32 pass)
     double *partial;      // [nseries][partial_pitch] sum of xhat^2 per CTA
     int partial_pitch, partial0;
     float *chunkmax;      // [nseries][chunkmax_pitch] max |xhat| per 16-slice step
@@ -74,6 +74,7 @@ bool tc_supported(const BeamformArgs &a);
 size_t tc_image_halfs(int S, int B);
 void tc_build_image(const double *w_re, const double *w_im, int S, int B, unsigned short *hi, unsigned short *lo);
 int launch_beamform_tc(const BeamformArgs &a, const void *wimg, cudaStream_t st);
+int tc_configure();                                     // opt in to the large dynamic shared memory (current device)
 int ippf_configure();                                   // opt in to the large dynamic shared memory
 int launch_trigger_reduce(const TriggerArgs &a, cudaStream_t st);   // sum e^2 + chunk max from the series
 int launch_trigger_finish(const TriggerArgs &a, cudaStream_t st);   // sigma, threshold scan, sort
@@ -92,8 +93,14 @@ struct lofar_plan {
     double kappa = 6.0;
     int env_window = 1;
     uint32_t max_cand = 65536;
+    // device memory: every plan-owned device buffer goes through these (lofar_plan_set_allocator)
+    void *(*alloc_fn)(size_t, void *) = nullptr;
+    void (*free_fn)(void *, void *) = nullptr;
+    void *alloc_ctx = nullptr;
+    size_t scratch_limit = (size_t)4 << 30;   // bytes of beam-sum scratch per time chunk
     // device state
     bool built = false;
+    bool reset_pending = false;        // carried state is zeroed on the stream of the next compute call
     int num_sms = 148;
     unsigned short *dWimg = nullptr;   // [K][2][image] fp16 hi/lo operand images for the tensor-core beamformer
     int tc_min_beams = 4;              // use tcgen05 from this many beams on (int8 input)

@@ -200,7 +200,7 @@ def test_error_paths(torch):
     X = torch.zeros(2 * 2 * 4 * 64 * 2 + 64, dtype=torch.int8, device="cuda")
     Z = torch.empty((1, 4, 64, 2), dtype=torch.float32, device="cuda")
     assert p.beamform_dedisperse(X, 0, Z, allow=range(8)) == binding.LOFAR_E_INVALID
-    assert p.beamform_dedisperse(X, 128, Z, allow=range(8)) == binding.LOFAR_E_SHAPE
+    assert p.beamform_dedisperse(X, 128, Z, allow=range(8)) == binding.LOFAR_E_STATE      # beyond max_slices
     assert p.beamform_dedisperse(X[1:], 64, Z, allow=range(8)) == binding.LOFAR_E_ALIGN
     assert p.beamform_dedisperse(X, 4, Z, allow=range(8)) == binding.LOFAR_E_ALIGN      # 8-byte row pitch
     assert p.beamform_dedisperse(X, 64, None, allow=range(8)) == binding.LOFAR_E_INVALID
