@@ -313,8 +313,7 @@ lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, int ztile
     a.gs = p->dGs; a.tw = p->dTw;
     a.partial = p->dPartial; a.partial_pitch = p->partial_pitch; a.partial0 = *partial0;
     a.chunkmax = p->dChunkMax; a.chunkmax_pitch = p->chunkmax_pitch; a.step0 = step0;
-    a.vec_ok = ((zpitch & 1) == 0) && ((reinterpret_cast<size_t>(Z) & 15) == 0) &&
-               (zpitch * (long long)p->K < (1LL << 32));   // 32-bit row offsets in the fast path
+    a.vec_ok = ((zpitch & 1) == 0) && ((reinterpret_cast<size_t>(Z) & 15) == 0);
     ProfScope prof(p, 1, st);
     const int n = launch_ippf(a, st);
     if (n < 0) return LOFAR_E_CUDA;

@@ -161,7 +161,7 @@ __global__ void __launch_bounds__(kBfThreads) beamform_kernel(BeamformArgs a)
                 for (int i = 0; i < NT; ++i) o[i] = acc[bb][i];
             }
             float2 *zr = a.Z + (size_t)((b0 + bb) * nph + d) * a.K * (size_t)a.zpitch +
-                         (a.ztile ? ((size_t)(col >> 5) * a.K + k) * 32 + (col & 31) : (size_t)k * a.zpitch + col);
+                         (a.ztile ? ((size_t)(col >> 4) * a.K + k) * 16 + (col & 15) : (size_t)k * a.zpitch + col);
             if (vec) {
 #pragma unroll
                 for (int i = 0; i < NT; i += 2)

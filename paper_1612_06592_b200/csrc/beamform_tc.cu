@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(kTcThreads) beamform_tc_kernel(TcArgs a)
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(mbar + 1);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int k = blockIdx.y;
+    const int k = blockIdx.x;           // sub-band fastest: CTAs running together write neighbouring lines of a Z tile
     const BeamformArgs &g = a.b;
 
     // weights image of this sub-band, zero the A tile once (pad stations stay zero)
@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(kTcThreads) beamform_tc_kernel(TcArgs a)
     const uint32_t sA_addr = smem_u32(sA), sB_addr = smem_u32(sB);
     const uint32_t lbo_b = (uint32_t)(a.np / 8) * 128;
 
-    const long long tile0 = (long long)blockIdx.x * a.tiles_per_cta;
+    const long long tile0 = (long long)blockIdx.y * a.tiles_per_cta;
     uint32_t phase = 0;
     for (int it = 0; it < a.tiles_per_cta; ++it) {
         const long long col0 = (tile0 + it) * 128;       // column in Z / offset inside this launch
@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(kTcThreads) beamform_tc_kernel(TcArgs a)
                     const int b = n0 / 2 + j;
                     if (b < g.B) {
                         float2 *zr = g.Z + (size_t)b * g.K * (size_t)g.zpitch +
-                                     (g.ztile ? ((size_t)(colt >> 5) * g.K + k) * 32 + (colt & 31)
+                                     (g.ztile ? ((size_t)(colt >> 4) * g.K + k) * 16 + (colt & 15)
                                               : (size_t)k * g.zpitch + colt);
                         *zr = make_float2(__uint_as_float(r[2 * j]), __uint_as_float(r[2 * j + 1]));
                     }
@@ -268,7 +268,7 @@ int launch_beamform_tc(const BeamformArgs &b, const void *wimg, cudaStream_t st)
     a.wimg = static_cast<const uint4 *>(wimg);
     const long long tiles = (b.nt + 127) / 128;
     a.tiles_per_cta = tiles < 32 ? (int)tiles : 32;
-    dim3 grid((unsigned)((tiles + a.tiles_per_cta - 1) / a.tiles_per_cta), (unsigned)b.K);
+    dim3 grid((unsigned)b.K, (unsigned)((tiles + a.tiles_per_cta - 1) / a.tiles_per_cta));
     const size_t smem = (size_t)a.kchunks * kLboA + 2 * (size_t)a.img16 * 16 + 16;
     beamform_tc_kernel<<<grid, kTcThreads, smem, st>>>(a);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;

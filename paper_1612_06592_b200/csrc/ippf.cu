@@ -3,18 +3,23 @@
 // transformation F^-1 y~ = y of the filtered signal" followed by the FIR system H; here one
 // application of the matched synthesis FIR g = 1024 h, reading A8).
 //
-// One CTA (512 threads, 16 warps) owns one series and marches along a span of time slices in
+// One CTA (512 threads, 16 warps, one per SM) owns one series and marches along a span of time slices in
 // steps of 16 slices:
-//   pre-pass : reads the K selected sub-band rows of Z for 16 slices (one 128-byte line per row),
-//              applies the trial phasor if asked, builds the packed half-spectrum V (fft_math.cuh)
-//              and stores it transposed -- slice-major -- into shared memory;
+//   stage    : the K selected sub-band rows of the step -- one 128-byte line per row -- are brought into a
+//              shared-memory stage by bulk asynchronous copies (cp.async.bulk + mbarrier; one copy of
+//              K*128 bytes from the plan's tiled scratch, one copy per row from a caller's Z), issued one
+//              step ahead so that they fly during the FFT and FIR of the current step;
+//   pre-pass : reads the stage, applies the trial phasor if asked, builds the packed half-spectrum V
+//              (fft_math.cuh) and stores it transposed -- slice-major -- into the current slice buffer;
 //   FFT      : warp w transforms slice w in place: a radix-16 and a radix-32 pass (fft512_warp);
-//   FIR      : thread n owns output residues r = 2n, 2n+1; the 31-slice window (15 carried + 16 new)
-//              is read from the previous and current slice buffers, the 16 taps from shared memory;
+//   FIR      : thread n owns output residues r = 2n, 2n+1 and keeps their 16 tap pairs in registers; the
+//              31-slice window (15 carried + 16 new) is read from the previous and current slice buffers;
 //              16 x 1024 contiguous output samples are written per step.
-// The 15-slice history lives in the "previous" shared-memory buffer, is loaded from the plan at the
-// start of a block and written back by the CTA that owns the last span; CTAs that start in the
-// middle of a block first transform the 16 slices before their span (no output).
+// Complex adds and the FIR run on the packed fp32x2 instructions (FADD2 / FFMA2): the same FMA-pipe
+// throughput as the scalar forms for half the issue slots (the kernel is issue-bound).
+// The 15-slice history lives in the "previous" buffer, is loaded from the plan at the start of a block and
+// written back by the CTA that owns the last span; CTAs that start in the middle of a block first
+// transform the 16 slices before their span (no output).
 #include "fft_math.cuh"
 #include "plan.h"
 
@@ -23,97 +28,116 @@ namespace {
 
 constexpr int kThreads = 512;
 constexpr int kTwCount = 256 + 512;        // w1024[256], TB[32][16] = exp(2 pi i j r / 512)
-constexpr size_t kSmemBytes = (size_t)(2 * kStep * kRow + kP * kH + kTwCount) * sizeof(float2) + 256;
+constexpr int kStageF2 = kH * kStep;       // stage: up to 512 rows x 16 slices of float2 = 64 KB
+constexpr size_t kSmemBytes = (size_t)(2 * kStep * kRow + kStageF2 + kTwCount) * sizeof(float2) + 256;
+
+typedef unsigned long long u64;
+
+// ---- packed fp32x2 helpers: a u64 is an aligned register pair (lo = .x, hi = .y) -------------------
+__device__ __forceinline__ u64 PK(float x, float y) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y)); return r; }
+__device__ __forceinline__ float LO(u64 v) { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v)); return x; }
+__device__ __forceinline__ float HI(u64 v) { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(v)); return y; }
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ u64 lds64(const float2 *p) { return *reinterpret_cast<const u64 *>(p); }
+__device__ __forceinline__ void sts64(float2 *p, u64 v) { *reinterpret_cast<u64 *>(p) = v; }
+// a * (c + i s), scalar products (a complex product needs the swapped pair, which the packed forms lack)
+__device__ __forceinline__ u64 cmulp(u64 a, float c, float s)
+{
+    const float ax = LO(a), ay = HI(a);
+    return PK(fmaf(c, ax, -s * ay), fmaf(c, ay, s * ax));
+}
+// a + i b and a - i b
+__device__ __forceinline__ u64 addi(u64 a, u64 b) { return PK(LO(a) - HI(b), HI(a) + LO(b)); }
+__device__ __forceinline__ u64 subi(u64 a, u64 b) { return PK(LO(a) + HI(b), HI(a) - LO(b)); }
+
+// ---- mbarrier + bulk asynchronous copy (TMA unit, SASS UBLKCP / SYNCS) ------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
 
 struct Ctx {
-    const float2 *Zs;      // rows of this series' beam (sub-band j at Zs + j*zpitch)
+    const float2 *Zs;      // this series' beam sums
     const float2 *ph;      // trial phasors of this series or nullptr
     long long zpitch, nc;
-    int K, k0, vec_ok, tiled;
+    int K, k0, bulk_rows, tiled;
 };
 
-// Two consecutive slices (col, col+1) of absolute sub-band k; zero outside the selected band / launch.
-__device__ __forceinline__ float4 load2(const Ctx &c, int k, long long col)
+// Brings the K rows x 16 slices of the step starting at slice q into the stage ([K][16] float2).
+// Returns true if the copy is asynchronous (completion on the mbarrier), false if the threads stored it.
+__device__ __forceinline__ bool stage_fill(const Ctx &c, long long q, float2 *stage, uint32_t bar, int tid)
 {
-    const int j = k - c.k0;
-    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (j < 0 || j >= c.K || col >= c.nc) return v;
-    const float2 *p = c.tiled ? c.Zs + ((size_t)(col >> 5) * c.K + j) * 32 + (col & 31)
-                              : c.Zs + (size_t)j * c.zpitch + col;
-    if (col + 1 < c.nc) {
-        if (c.vec_ok) {
-            v = __ldcs(reinterpret_cast<const float4 *>(p));
-        } else {
-            float2 z0 = p[0], z1 = p[1];
-            v = make_float4(z0.x, z0.y, z1.x, z1.y);
+    if (c.tiled) {
+        // plan scratch [tile = q/16][K][16]: the whole step is one contiguous block
+        if (tid == 0) {
+            const uint32_t bytes = (uint32_t)c.K * 128u;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the stage was last read by ordinary loads
+            mbar_arrive_expect_tx(bar, bytes);
+            bulk_g2s(smem_u32(stage), c.Zs + (size_t)(q >> 4) * c.K * 16, bytes, bar);
         }
-    } else {
-        float2 z0 = p[0];
-        v.x = z0.x; v.y = z0.y;
+        return true;
     }
-    return v;
+    if (c.bulk_rows && q + kStep <= c.nc) {
+        // caller's Z [K][zpitch]: one 128-byte line per row
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        if (tid == 0) mbar_arrive_expect_tx(bar, (uint32_t)c.K * 128u);
+        for (int j = tid; j < c.K; j += kThreads)
+            bulk_g2s(smem_u32(stage + j * kStep), c.Zs + (size_t)j * c.zpitch + q, 128u, bar);
+        return true;
+    }
+    // ragged or unaligned: plain loads, zero beyond the end of the launch
+    for (int idx = tid; idx < c.K * kStep; idx += kThreads) {
+        const int j = idx >> 4, t = idx & 15;
+        float2 v = make_float2(0.f, 0.f);
+        if (q + t < c.nc) v = c.Zs[(size_t)j * c.zpitch + q + t];
+        stage[idx] = v;
+    }
+    return false;
 }
 
-// Global loads of one 16-slice step, held in registers so that they can be issued one step ahead:
-// thread unit i covers conjugate pair m = (tid>>3) + 64 i (m = 0: bins 0 and 256) and slices 2tp, 2tp+1.
-struct StepRegs { float4 a[4], b[4]; };
-
-__device__ __forceinline__ void prefetch(const Ctx &c, long long q, int tid, StepRegs &r)
-{
-    const int tp = tid & 7, m0 = tid >> 3;
-    const long long col = q + 2 * tp;
-    if (c.vec_ok && col + 1 < c.nc) {
-        // common case, branch-free: predicated 16-byte loads, rows outside the selected band read as zero
-        // tiled scratch: 32-slice tiles [K][32]: a step reads 128 of every 256 bytes of one contiguous block; else rows zpitch apart
-        const float2 *p0 = c.tiled ? c.Zs + (size_t)(col >> 5) * c.K * 32 + (col & 31) : c.Zs + col;
-        const unsigned K = (unsigned)c.K, zp = c.tiled ? 32u : (unsigned)c.zpitch;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int m = m0 + 64 * i;
-            const unsigned ja = (unsigned)(m - c.k0), jb = (unsigned)((m == 0 ? 256 : 512 - m) - c.k0);
-            float4 va = make_float4(0.f, 0.f, 0.f, 0.f), vb = va;
-            if (ja < K) va = __ldcs(reinterpret_cast<const float4 *>(p0 + (size_t)(ja * zp)));
-            if (jb < K) vb = __ldcs(reinterpret_cast<const float4 *>(p0 + (size_t)(jb * zp)));
-            r.a[i] = va; r.b[i] = vb;
-        }
-        // pull the rows of the step after this one into L2 (one 128-byte line per row: lanes with tp == 0)
-        if (tp == 0 && col + 2 * kStep < c.nc) {
-            const float2 *p1 = c.tiled ? c.Zs + (size_t)((col + kStep) >> 5) * c.K * 32 + ((col + kStep) & 31) : p0 + kStep;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int m = m0 + 64 * i;
-                const unsigned ja = (unsigned)(m - c.k0), jb = (unsigned)((m == 0 ? 256 : 512 - m) - c.k0);
-                if (ja < K) asm volatile("prefetch.global.L2 [%0];" :: "l"(p1 + (size_t)(ja * zp)));
-                if (jb < K) asm volatile("prefetch.global.L2 [%0];" :: "l"(p1 + (size_t)(jb * zp)));
-            }
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-            const int m = m0 + 64 * i;
-            r.a[i] = load2(c, m, col);
-            r.b[i] = load2(c, m == 0 ? 256 : 512 - m, col);
-        }
-    }
-}
-
-// Pre-pass of the 16 slices held in r into dst[16][kRow] (packed half-spectrum V, slice-major).
 __device__ __forceinline__ float4 rotate2(float4 v, float2 f)
 {
     return make_float4(f.x * v.x - f.y * v.y, f.x * v.y + f.y * v.x, f.x * v.z - f.y * v.w, f.x * v.w + f.y * v.z);
 }
 
-__device__ __forceinline__ void prepass(const Ctx &c, const StepRegs &r, float2 *dst, const float2 *stw, int tid)
+// Pre-pass of the 16 staged slices into dst[16][kRow] (packed half-spectrum V, slice-major).
+// Thread unit i covers the conjugate pair m = (tid>>3) + 64 i (m = 0: bins 0 and 256) and slices 2tp, 2tp+1.
+//   P = a + conj(b), D = a - conj(b), U' = (Im(wD), Re(wD));  V[m] = (P.x - U'.x, P.y + U'.y),
+//   V[512-m] = (P.x + U'.x, U'.y - P.y)            (fft_math.cuh: prepass_pair, restated for packed ops)
+__device__ __forceinline__ void prepass(const Ctx &c, const float2 *stage, float2 *dst, const float2 *stw, int tid)
 {
     const int tp = tid & 7, m0 = tid >> 3;
     float2 *r0 = dst + 2 * tp * kRow, *r1 = r0 + kRow;
+    const u64 pm = PK(1.f, -1.f), mp = PK(-1.f, 1.f);
+    const float4 *st4 = reinterpret_cast<const float4 *>(stage) + tp;      // + 8 float4 per row
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         const int m = m0 + 64 * i;
-        float4 a = r.a[i], b = r.b[i];
+        const unsigned ja = (unsigned)(m - c.k0), jb = (unsigned)((m == 0 ? 256 : 512 - m) - c.k0);
+        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+        if (ja < (unsigned)c.K) a = st4[ja * 8];
+        if (jb < (unsigned)c.K) b = st4[jb * 8];
         if (c.ph) {
             // STEC trial fan-out (a2): the trial's phasor multiplies the beam sums as they enter the transform
-            const unsigned ja = (unsigned)(m - c.k0), jb = (unsigned)((m == 0 ? 256 : 512 - m) - c.k0);
             if (ja < (unsigned)c.K) a = rotate2(a, __ldg(c.ph + ja));
             if (jb < (unsigned)c.K) b = rotate2(b, __ldg(c.ph + jb));
         }
@@ -124,13 +148,63 @@ __device__ __forceinline__ void prepass(const Ctx &c, const StepRegs &r, float2 
             r1[pad(256)] = prepass_quarter(make_float2(b.z, b.w));
         } else {
             const float2 w = stw[m];
-            float2 vm, vmir;
-            prepass_pair(make_float2(a.x, a.y), make_float2(b.x, b.y), w, vm, vmir);
-            r0[pad(m)] = vm; r0[pad(512 - m)] = vmir;
-            prepass_pair(make_float2(a.z, a.w), make_float2(b.z, b.w), w, vm, vmir);
-            r1[pad(m)] = vm; r1[pad(512 - m)] = vmir;
+            const int im = pad(m), imir = pad(512 - m);
+            {
+                const u64 A = PK(a.x, a.y), B = PK(b.x, b.y);
+                const u64 P = fma2(B, pm, A), D = fma2(B, mp, A);
+                const float dx = LO(D), dy = HI(D);
+                const u64 U = PK(fmaf(w.x, dy, w.y * dx), fmaf(w.x, dx, -w.y * dy));
+                sts64(r0 + im, fma2(U, mp, P));
+                sts64(r0 + imir, fma2(P, pm, U));
+            }
+            {
+                const u64 A = PK(a.z, a.w), B = PK(b.z, b.w);
+                const u64 P = fma2(B, pm, A), D = fma2(B, mp, A);
+                const float dx = LO(D), dy = HI(D);
+                const u64 U = PK(fmaf(w.x, dy, w.y * dx), fmaf(w.x, dx, -w.y * dy));
+                sts64(r1 + im, fma2(U, mp, P));
+                sts64(r1 + imir, fma2(P, pm, U));
+            }
         }
     }
+}
+
+// Inverse 8-point DFT in place on packed complex values: x[m] <- sum_r x[r] exp(+2 pi i r m / 8).
+__device__ __forceinline__ void idft8p(u64 *x)
+{
+    const float s = 0.70710678118654752440f;
+    const u64 a0 = add2(x[0], x[4]), a1 = sub2(x[0], x[4]);
+    const u64 a2 = add2(x[2], x[6]), a3 = sub2(x[2], x[6]);
+    const u64 e0 = add2(a0, a2), e2 = sub2(a0, a2), e1 = addi(a1, a3), e3 = subi(a1, a3);
+    const u64 b0 = add2(x[1], x[5]), b1 = sub2(x[1], x[5]);
+    const u64 b2 = add2(x[3], x[7]), b3 = sub2(x[3], x[7]);
+    const u64 o0 = add2(b0, b2), o2 = sub2(b0, b2), o1 = addi(b1, b3), o3 = subi(b1, b3);
+    // odd part times W8^m = exp(+i pi m / 4):  o1 (1+i)/sqrt2 = s (x - y, x + y);  o3 (-1+i)/sqrt2 = s (-(x + y), x - y)
+    const u64 q1 = PK(LO(o1) - HI(o1), LO(o1) + HI(o1));
+    const u64 q3 = PK(LO(o3) + HI(o3), LO(o3) - HI(o3));
+    x[0] = add2(e0, o0); x[4] = sub2(e0, o0);
+    x[1] = fma2(q1, PK(s, s), e1); x[5] = fma2(q1, PK(-s, -s), e1);
+    x[2] = addi(e2, o2); x[6] = subi(e2, o2);
+    x[3] = fma2(q3, PK(-s, s), e3); x[7] = fma2(q3, PK(s, -s), e3);
+}
+
+// Inverse 16-point DFT in place (two 8-point DFTs of the even / odd inputs, then the W16^m butterflies).
+__device__ __forceinline__ void idft16p(u64 *x)
+{
+    u64 e[8], o[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { e[i] = x[2 * i]; o[i] = x[2 * i + 1]; }
+    idft8p(e);
+    idft8p(o);
+    const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f, h = 0.70710678118654752440f;
+    x[0] = add2(e[0], o[0]); x[8] = sub2(e[0], o[0]);
+    { const u64 t = cmulp(o[1], c1, s1); x[1] = add2(e[1], t); x[9] = sub2(e[1], t); }
+    { const u64 q = PK(LO(o[2]) - HI(o[2]), LO(o[2]) + HI(o[2])); x[2] = fma2(q, PK(h, h), e[2]); x[10] = fma2(q, PK(-h, -h), e[2]); }
+    { const u64 t = cmulp(o[3], s1, c1); x[3] = add2(e[3], t); x[11] = sub2(e[3], t); }
+    x[4] = addi(e[4], o[4]); x[12] = subi(e[4], o[4]);
+    { const u64 t = cmulp(o[5], -s1, c1); x[5] = add2(e[5], t); x[13] = sub2(e[5], t); }
+    { const u64 q = PK(LO(o[6]) + HI(o[6]), LO(o[6]) - HI(o[6])); x[6] = fma2(q, PK(-h, h), e[6]); x[14] = fma2(q, PK(h, -h), e[6]); }
+    { const u64 t = cmulp(o[7], -c1, s1); x[7] = add2(e[7], t); x[15] = sub2(e[7], t); }
 }
 
 // 512-point inverse complex FFT of one slice row by one warp, in place: 512 = 16 x 32.
@@ -140,18 +214,21 @@ __device__ __forceinline__ void prepass(const Ctx &c, const StepRegs &r, float2 
 //           W32^m, the halves are exchanged with shuffles; outputs go to j + 16 m (m < 16 low lane, m >= 16 high).
 __device__ __forceinline__ void fft512_warp(float2 *row, const float2 *stw, int lane)
 {
-    float2 x[16];
+    u64 x[16];
 #pragma unroll
-    for (int r = 0; r < 16; ++r) x[r] = row[pad(lane + 32 * r)];
-    idft16(x);
+    for (int r = 0; r < 16; ++r) x[r] = lds64(row + pad(lane + 32 * r));
+    idft16p(x);
     __syncwarp();
 #pragma unroll
-    for (int m = 0; m < 16; ++m) row[pad(16 * lane + m)] = x[m];
+    for (int m = 0; m < 16; ++m) sts64(row + pad(16 * lane + m), x[m]);
     __syncwarp();
     const float2 *T = stw + 256 + lane;          // T[32 r' + lane] = exp(2 pi i j (hh + 2 r') / 512)
 #pragma unroll
-    for (int r = 0; r < 16; ++r) x[r] = cmul(row[pad(lane + 32 * r)], T[32 * r]);
-    idft16(x);
+    for (int r = 0; r < 16; ++r) {
+        const float2 t = T[32 * r];
+        x[r] = cmulp(lds64(row + pad(lane + 32 * r)), t.x, t.y);
+    }
+    idft16p(x);
     const bool hi = lane >= 16;
     if (hi) {
         // W32^m = exp(2 pi i m / 32), m = 0..15
@@ -166,31 +243,63 @@ __device__ __forceinline__ void fft512_warp(float2 *row, const float2 *stw, int 
                               0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
                               0.38268343236508977173f, 0.19509032201612826785f};
 #pragma unroll
-        for (int m = 1; m < 16; ++m) x[m] = cmul(x[m], make_float2(c[m], sn[m]));
+        for (int m = 1; m < 16; ++m) x[m] = cmulp(x[m], c[m], sn[m]);
     }
+    // low lane: E + O', high lane: E - O'  ==  other + sg * own with sg = +1 / -1
+    const u64 sg = hi ? PK(-1.f, -1.f) : PK(1.f, 1.f);
 #pragma unroll
     for (int m = 0; m < 16; ++m) {
-        float2 other;
-        other.x = __shfl_xor_sync(0xffffffffu, x[m].x, 16);
-        other.y = __shfl_xor_sync(0xffffffffu, x[m].y, 16);
-        x[m] = hi ? csub(other, x[m]) : cadd(x[m], other);     // low lane: E + O', high lane: E - O'
+        const u64 other = __shfl_xor_sync(0xffffffffu, x[m], 16);
+        x[m] = fma2(x[m], sg, other);
     }
     __syncwarp();
     const int base = (lane & 15) + (hi ? 256 : 0);
 #pragma unroll
-    for (int m = 0; m < 16; ++m) row[pad(base + 16 * m)] = x[m];
+    for (int m = 0; m < 16; ++m) sts64(row + pad(base + 16 * m), x[m]);
     __syncwarp();
+}
+
+// Synthesis FIR of one step: out[j] = sum_t g[t] * win[15 + j - t], j = 0..15, window = prev rows 1..15 + cur rows
+// 0..15, column pn; FULL = all 16 output slices valid (no predicates on the fast path).
+template <bool FULL>
+__device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, const u64 (&g)[kP], int pn, float *out,
+                                         int tid, int nvalid, u64 &ssum2, float &smax)
+{
+    u64 acc[kStep];
+#pragma unroll
+    for (int j = 0; j < kStep; ++j) acc[j] = 0ull;
+#pragma unroll
+    for (int i = 0; i < kP - 1 + kStep; ++i) {
+        const u64 x = lds64((i < kP - 1) ? prev + (i + 1) * kRow + pn : cur + (i - (kP - 1)) * kRow + pn);
+#pragma unroll
+        for (int t = 0; t < kP; ++t) {
+            const int j = i - (kP - 1) + t;
+            if (j >= 0 && j < kStep) acc[j] = fma2(g[t], x, acc[j]);
+        }
+        // output slice j = i - 15 is complete once window element i has been applied: store it now so
+        // that the 64 KB of stores per step are spread over the second half of the FIR
+        if (i >= kP - 1) {
+            const int j = i - (kP - 1);
+            if (FULL || j < nvalid) {
+                const float vx = LO(acc[j]), vy = HI(acc[j]);
+                if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)j * kM + 2 * tid), make_float2(vx, vy));
+                ssum2 = fma2(acc[j], acc[j], ssum2);
+                smax = fmaxf(smax, fmaxf(fabsf(vx), fabsf(vy)));
+            }
+        }
+    }
 }
 
 __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2 *buf0 = reinterpret_cast<float2 *>(smem_raw);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *stage = reinterpret_cast<float2 *>(smem_raw);          // [K][16], 128-byte aligned for the bulk copies
+    float2 *buf0 = stage + kStageF2;
     float2 *buf1 = buf0 + kStep * kRow;
-    float2 *sg = buf1 + kStep * kRow;      // [16][512]
-    float2 *stw = sg + kP * kH;            // [kTwCount]
-    float *sred = reinterpret_cast<float *>(stw + kTwCount);   // 16 floats + 16 doubles (aligned)
-    double *sdred = reinterpret_cast<double *>(sred + 32);
+    float2 *stw = buf1 + kStep * kRow;                             // [kTwCount]
+    float *sred = reinterpret_cast<float *>(stw + kTwCount);       // 16 floats, 16 doubles, the mbarrier
+    double *sdred = reinterpret_cast<double *>(sred + 16);
+    const uint32_t bar = smem_u32(sdred + 16);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int series = blockIdx.x % a.nseries;
@@ -204,100 +313,79 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     const int zi = a.zmap_trials ? series / a.zmap_trials : series;
     c.Zs = a.Z + (size_t)zi * a.K * (size_t)a.zpitch;
     c.ph = a.zmap_trials ? a.Dph + (size_t)(series % a.zmap_trials) * a.K : nullptr;
-    c.zpitch = a.zpitch; c.nc = a.nc; c.K = a.K; c.k0 = a.k0; c.vec_ok = a.vec_ok; c.tiled = a.ztile;
+    c.zpitch = a.zpitch; c.nc = a.nc; c.K = a.K; c.k0 = a.k0; c.bulk_rows = a.vec_ok; c.tiled = a.ztile;
 
-    for (int i = tid; i < kP * kH; i += kThreads) sg[i] = a.gs[i];
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     for (int i = tid; i < kTwCount; i += kThreads) stw[i] = a.tw[i];
+    u64 g[kP];                                   // the 16 tap pairs of residues 2 tid, 2 tid + 1, for the whole span
+#pragma unroll
+    for (int t = 0; t < kP; ++t) { const float2 v = __ldg(a.gs + t * kH + tid); g[t] = PK(v.x, v.y); }
+    const int pn = pad(tid);
 
     float2 *prev = buf0, *cur = buf1;
     if (span == 0) {
         const float *h = a.hist_in + (size_t)series * (kP - 1) * kM;
 #pragma unroll
         for (int i = 0; i < kP - 1; ++i)
-            prev[(i + 1) * kRow + pad(tid)] = *reinterpret_cast<const float2 *>(h + (size_t)i * kM + 2 * tid);
-        __syncthreads();
-    } else {
-        __syncthreads();   // twiddles visible
-        StepRegs w;
-        prefetch(c, qs - kStep, tid, w);
-        prepass(c, w, cur, stw, tid);
-        __syncthreads();
-        fft512_warp(cur + warp * kRow, stw, lane);
-        __syncthreads();
-        float2 *t = prev; prev = cur; cur = t;
+            prev[(i + 1) * kRow + pn] = *reinterpret_cast<const float2 *>(h + (size_t)i * kM + 2 * tid);
     }
-    StepRegs regs;
-    prefetch(c, qs, tid, regs);
+    __syncthreads();                             // mbarrier, twiddles and history visible
+
+    // the first step of a span that starts inside the block is a warm-up: transform the 16 slices before it
+    const long long q_first = span == 0 ? qs : qs - kStep;
+    uint32_t phase = 0;
+    bool async = stage_fill(c, q_first, stage, bar, tid);
 
     float *out = a.series ? a.series + (size_t)series * a.series_pitch + a.out0 : nullptr;
     double dsum = 0.0;
 
-    for (long long q = qs; q < qe; q += kStep) {
-        const int nvalid = (qe - q < kStep) ? (int)(qe - q) : kStep;
-        prepass(c, regs, cur, stw, tid);
-        if (q + kStep < qe) prefetch(c, q + kStep, tid, regs);   // next step's loads fly during FFT + FIR
-        __syncthreads();
+    for (long long q = q_first; q < qe; q += kStep) {
+        if (async) { while (!mbar_try_wait(bar, phase)) {} phase ^= 1; }
+        else __syncthreads();
+        prepass(c, stage, cur, stw, tid);
+        __syncthreads();                         // cur complete, stage free
+        if (q + kStep < qe) async = stage_fill(c, q + kStep, stage, bar, tid);   // flies during FFT + FIR
         fft512_warp(cur + warp * kRow, stw, lane);
         __syncthreads();
 
-        // ---- synthesis FIR: out[j] = sum_t g[t] * win[15 + j - t] ----
-        float2 g[kP], acc[kStep];
+        if (q >= qs) {
+            const int nvalid = (qe - q < kStep) ? (int)(qe - q) : kStep;
+            u64 ssum2 = 0ull;
+            float smax = 0.f;
+            float *o = out ? out + (size_t)q * kM : nullptr;
+            if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
+            else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
+            dsum += (double)(LO(ssum2) + HI(ssum2));
 #pragma unroll
-        for (int t = 0; t < kP; ++t) g[t] = sg[t * kH + tid];
-#pragma unroll
-        for (int j = 0; j < kStep; ++j) acc[j] = make_float2(0.f, 0.f);
-        const int pn = pad(tid);
-        float ssum = 0.f, smax = 0.f;
-#pragma unroll
-        for (int i = 0; i < kP - 1 + kStep; ++i) {
-            const float2 x = (i < kP - 1) ? prev[(i + 1) * kRow + pn] : cur[(i - (kP - 1)) * kRow + pn];
-#pragma unroll
-            for (int t = 0; t < kP; ++t) {
-                const int j = i - (kP - 1) + t;
-                if (j >= 0 && j < kStep) {
-                    acc[j].x = fmaf(g[t].x, x.x, acc[j].x);
-                    acc[j].y = fmaf(g[t].y, x.y, acc[j].y);
-                }
-            }
-            // output slice j = i - 15 is complete once window element i has been applied: store it now so
-            // that the 64 KB of stores per step are spread over the second half of the FIR
-            if (i >= kP - 1) {
-                const int j = i - (kP - 1);
-                if (j < nvalid) {
-                    if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)(q + j) * kM + 2 * tid), acc[j]);
-                    ssum = fmaf(acc[j].x, acc[j].x, ssum);
-                    ssum = fmaf(acc[j].y, acc[j].y, ssum);
-                    smax = fmaxf(smax, fmaxf(fabsf(acc[j].x), fabsf(acc[j].y)));
-                }
-            }
-        }
-        dsum += (double)ssum;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, o));
-        if (lane == 0) sred[warp] = smax;
+            for (int s = 16; s > 0; s >>= 1) smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, s));
+            if (lane == 0) sred[warp] = smax;
 
-        if (is_last && q + kStep >= qe) {
-            // carry the last 15 valid slices: relative slice i = nvalid-15 .. nvalid-1 of this step
-            float *h = a.hist_out + (size_t)series * (kP - 1) * kM;
-            for (int idx = 0; idx < kP - 1; ++idx) {
-                const int i = nvalid - (kP - 1) + idx;
-                const float2 v = (i < 0) ? prev[(kStep + i) * kRow + pn] : cur[i * kRow + pn];
-                *reinterpret_cast<float2 *>(h + (size_t)idx * kM + 2 * tid) = v;
+            if (is_last && q + kStep >= qe) {
+                // carry the last 15 valid slices: relative slice i = nvalid-15 .. nvalid-1 of this step
+                float *h = a.hist_out + (size_t)series * (kP - 1) * kM;
+                for (int idx = 0; idx < kP - 1; ++idx) {
+                    const int i = nvalid - (kP - 1) + idx;
+                    const float2 v = (i < 0) ? prev[(kStep + i) * kRow + pn] : cur[i * kRow + pn];
+                    *reinterpret_cast<float2 *>(h + (size_t)idx * kM + 2 * tid) = v;
+                }
             }
-        }
-        __syncthreads();
-        if (tid == 0) {
-            float m = sred[0];
+            __syncthreads();
+            if (tid == 0) {
+                float m = sred[0];
 #pragma unroll
-            for (int w = 1; w < kThreads / 32; ++w) m = fmaxf(m, sred[w]);
-            a.chunkmax[(size_t)series * a.chunkmax_pitch + a.step0 + q / kStep] = m;
+                for (int w = 1; w < kThreads / 32; ++w) m = fmaxf(m, sred[w]);
+                a.chunkmax[(size_t)series * a.chunkmax_pitch + a.step0 + q / kStep] = m;
+            }
         }
         float2 *t = prev; prev = cur; cur = t;
     }
 
     // per-CTA sum of squares, fixed reduction order
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) dsum += __shfl_xor_sync(0xffffffffu, dsum, o);
+    for (int s = 16; s > 0; s >>= 1) dsum += __shfl_xor_sync(0xffffffffu, dsum, s);
     if (lane == 0) sdred[warp] = dsum;
     __syncthreads();
     if (tid == 0) {

@@ -17,7 +17,7 @@ struct BeamformArgs {
     long long nt;         // slices to process
     float2 *Z;            // [nz][K][zpitch], slice t0+i stored at column i
     long long zpitch;
-    int ztile;            // 1: plan scratch layout [nz][zpitch/32][K][32] (32-slice tiles contiguous over sub-bands)
+    int ztile;            // 1: plan scratch layout [nz][zpitch/16][K][16] (16-slice tiles contiguous over sub-bands)
     const float2 *W;      // [K][B][S] weights (de-dispersion phase folded in when D == 1)
     const float2 *Dph;    // [D][K] trial phasors, used when nphase > 0
     int S, K, B;
@@ -28,7 +28,7 @@ struct BeamformArgs {
 struct IppfArgs {
     const float2 *Z;      // [nz][K][zpitch]
     long long zpitch;
-    int ztile;            // 1: [nz][zpitch/32][K][32]
+    int ztile;            // 1: [nz][zpitch/16][K][16]: one step of one series is one contiguous K*128-byte block
     long long nc;         // slices in this launch (columns 0..nc-1 of Z)
     float *series;        // [nseries][series_pitch]; this launch writes samples out0 .. out0 + nc*1024
     long long series_pitch;
@@ -45,7 +45,7 @@ struct IppfArgs {
     int partial_pitch, partial0;
     float *chunkmax;      // [nseries][chunkmax_pitch] max |xhat| per 16-slice step
     long long chunkmax_pitch, step0;
-    int vec_ok;           // Z rows allow 16-byte loads
+    int vec_ok;           // Z rows are 16-byte aligned at every step start (128-byte bulk copies allowed)
 };
 
 struct TriggerArgs {
