@@ -291,3 +291,58 @@ ORACLE_API long long lofar_oracle_candidates(const double *env, const double *si
     }
     return count;
 }
+
+/* ===========================================================================
+ * Rows "next" of SURVEY.md section 8(f).  Same rules as above: plain, slow,
+ * double precision, no code shared with the CUDA library.
+ * =========================================================================== */
+
+/* ---------------------------------------------------------------------------
+ * O9  Causal sigma (f3; the ns-resolution signal is used "only
+ * to trigger the read-out", so the threshold has to be known while the block
+ * is being reconstructed).  Reading A21: the reference level of
+ * block i is the envelope RMS of block i-1 of the same series,
+ *   sigma_ref_i[s] = sigma_{i-1}[s]  (i >= 1),
+ *   sigma_ref_0[s] = sigma_init[s] if the caller gave one, else sigma_0[s]
+ *                    (the first block of a stream is its own reference),
+ * and O8 is applied with sigma_ref in place of sigma.  The arithmetic of this
+ * definition is O7 + O8 with another sigma argument; the state (sigma of the
+ * previous block) is carried by the caller (oracle/lofar_oracle.py).
+ * ------------------------------------------------------------------------- */
+
+/* ---------------------------------------------------------------------------
+ * O10  Time clustering of candidates into events (f3; what a read-out request
+ * of the transient buffers needs).  Reading A22: input is the
+ * candidate list of ONE block, one beam after the other, samples increasing
+ * (O8's output order).  Consecutive candidates of the same beam belong to the
+ * same event iff their samples differ by at most `gap`.  Per event:
+ *   first, last sample; number of candidates; the peak = the candidate with
+ *   the largest snr = env/sigma (the lowest sample on exact ties).
+ * beam[n], sample[n], snr[n]: inputs.  ev_first/ev_last/ev_count/ev_peak
+ * (index into the input list): outputs, capacity cap.  Returns the number of
+ * events.
+ * ------------------------------------------------------------------------- */
+ORACLE_API long long lofar_oracle_cluster(const int *beam, const long long *sample, const double *snr,
+                                          long long n, long long gap, long long cap,
+                                          long long *ev_first, long long *ev_last, long long *ev_count,
+                                          long long *ev_peak)
+{
+    long long nev = 0;
+    long long i = 0;
+    while (i < n) {
+        long long j = i, peak = i;
+        while (j + 1 < n && beam[j + 1] == beam[i] && sample[j + 1] - sample[j] <= gap) {
+            ++j;
+            if (snr[j] > snr[peak]) peak = j;
+        }
+        if (nev < cap) {
+            ev_first[nev] = sample[i];
+            ev_last[nev] = sample[j];
+            ev_count[nev] = j - i + 1;
+            ev_peak[nev] = peak;
+        }
+        ++nev;
+        i = j + 1;
+    }
+    return nev;
+}
