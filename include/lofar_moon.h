@@ -69,6 +69,22 @@ typedef struct {
     float sigma;     /* sigma of that series over this block                       */
 } lofar_candidate;
 
+/* One event = a run of candidates of one beam whose samples differ by at most `gap` (48 bytes;
+ * reading A22 in DESIGN.md). */
+typedef struct {
+    uint32_t beam;          /* series / D                                              */
+    uint32_t count;         /* candidates merged into the event                        */
+    uint64_t first_sample;  /* global 5 ns index of the first and                      */
+    uint64_t last_sample;   /* ... the last candidate                                  */
+    uint64_t peak_sample;   /* the candidate with the largest env/sigma                */
+    uint32_t peak_trial;    /* (lowest sample on exact ties), its trial,               */
+    float peak_env;         /* envelope,                                               */
+    float peak_sigma;       /* reference level                                         */
+    float peak_snr;         /* and env/sigma                                           */
+} lofar_event;
+
+typedef enum { LOFAR_SIGMA_BLOCK = 0, LOFAR_SIGMA_CAUSAL = 1 } lofar_sigma_mode;
+
 /* ---- plan ---------------------------------------------------------------------------------
  * BASELINE.json:north_star: "lofar_plan_create(stations, subbands, beams, taps, STEC)".
  * Creates a plan with one trial (D = 1) at stec_tecu, sub-bands k0 = 0..subbands-1 until
@@ -101,6 +117,17 @@ LOFAR_API lofar_status lofar_plan_set_input(lofar_plan *plan, lofar_dtype dtype,
  * (e[n] = sqrt(mean of xhat[n-W+1..n]^2), reading A13), candidate buffer capacity. */
 LOFAR_API lofar_status lofar_plan_set_trigger(lofar_plan *plan, double kappa, int env_window,
                                               uint32_t max_candidates);
+/* Reference level of the trigger (the recovered signal is used "only
+ * to trigger the read-out", so the threshold must be known while a block is reconstructed).
+ * LOFAR_SIGMA_BLOCK (default): candidates of a block are measured against the envelope RMS of that
+ * block (reading A14).  LOFAR_SIGMA_CAUSAL: block i is measured against sigma of block i-1 of the same
+ * series (reading A21); the first block after a reset uses sigma_init_host[B*D] if not NULL, else its own
+ * sigma.  With the level known in advance the candidates are decided in the inverse-PPF epilogue and
+ * lofar_run_block / lofar_stream_push need not write the series (series == NULL).  `sigma` outputs always
+ * receive the RMS of the current block; candidate records carry the level they were measured against.
+ * Causal mode needs env_window 1 (LOFAR_E_INVALID otherwise, from the compute calls). */
+LOFAR_API lofar_status lofar_plan_set_sigma_mode(lofar_plan *plan, lofar_sigma_mode mode,
+                                                 const float *sigma_init_host);
 /* Device bytes the plan allocates for the current settings: tables (weights, tensor-core operand
  * images, trial phasors, taps, twiddles), 2 x carried history, envelope tail, beam-sum scratch,
  * trigger partials, and the two streaming staging slots (input block, candidates, count, sigma)
@@ -146,10 +173,24 @@ LOFAR_API lofar_status lofar_inverse_ppf(lofar_plan *plan, const void *Z, int sl
 LOFAR_API lofar_status lofar_trigger(lofar_plan *plan, const float *series, int slices,
                                      lofar_candidate *cand, uint32_t *count, float *sigma,
                                      void *stream);
-/* The whole chain on one block: a1..a5 with the beam sums kept in plan scratch. */
+/* The whole chain on one block: a1..a5 with the beam sums kept in plan scratch.
+ * series == NULL selects the trigger-only mode: nothing of the 5 ns series is written
+ * to HBM; sigma and the candidate list are the same as with a series (same definitions; values within
+ * fp32 rounding).  With LOFAR_SIGMA_BLOCK the chunks whose maximum can reach kappa*sigma are recomputed
+ * from X after sigma is known (X must stay valid until the call's work has completed, as always); with
+ * LOFAR_SIGMA_CAUSAL candidates come out of the first pass.  Needs env_window 1.  With D > 1 and more
+ * raw threshold crossings than max_candidates, *count is that raw number (an overflow), not the number of
+ * distinct (beam, sample) candidates. */
 LOFAR_API lofar_status lofar_run_block(lofar_plan *plan, const void *X, int slices, float *series,
                                        lofar_candidate *cand, uint32_t *count, float *sigma,
                                        void *stream);
+
+/* f3: groups a candidate list as produced by lofar_trigger / lofar_run_block (device pointers, sorted by
+ * (beam, sample), *count valid) into events: consecutive candidates of one beam whose samples differ by at
+ * most gap_samples.  *nevents receives the number of events, the first max_events are stored in order. */
+LOFAR_API lofar_status lofar_cluster(lofar_plan *plan, const lofar_candidate *cand, const uint32_t *count,
+                                     uint64_t gap_samples, lofar_event *events, uint32_t *nevents,
+                                     uint32_t max_events, void *stream);
 
 /* ---- streaming driver (a6; BASELINE.json:configs[4]) -------------------------------------------
  * lofar_stream_reset: waits for the plan's own streams and resets the stream offset; the carried
@@ -159,7 +200,7 @@ LOFAR_API lofar_status lofar_run_block(lofar_plan *plan, const void *X, int slic
  * buffers on a copy stream while the previous block computes on a compute stream; then
  * lofar_run_block runs on it; then count, sigma[B*D] and the stored candidates are copied to
  * the *_host buffers (any of which may be NULL).  series is a device buffer (never copied to
- * the host).  Returns without waiting.  Host result buffers and X_host must stay untouched
+ * the host) or NULL (trigger-only, see lofar_run_block).  Returns without waiting.  Host result buffers and X_host must stay untouched
  * until lofar_stream_sync returns.
  * lofar_stream_sync: blocks until all pushed blocks are done; returns LOFAR_E_OVERFLOW if any
  * block since the last sync had more candidates than max_candidates. */

@@ -17,16 +17,23 @@ LIB_PATH = os.path.join(_HERE, "liblofar_moon.so")
 LOFAR_OK, LOFAR_E_INVALID, LOFAR_E_SHAPE, LOFAR_E_ALIGN, LOFAR_E_ALLOC, LOFAR_E_CUDA, \
     LOFAR_E_OVERFLOW, LOFAR_E_STATE = range(8)
 LOFAR_CI8, LOFAR_CI16 = 0, 1
+LOFAR_SIGMA_BLOCK, LOFAR_SIGMA_CAUSAL = 0, 1
 
 # numpy view of lofar_candidate (24 bytes)
 CANDIDATE_DTYPE = np.dtype([("series", "<u4"), ("trial", "<u4"), ("sample", "<u8"),
                             ("env", "<f4"), ("sigma", "<f4")])
 assert CANDIDATE_DTYPE.itemsize == 24
+# numpy view of lofar_event (48 bytes)
+EVENT_DTYPE = np.dtype([("beam", "<u4"), ("count", "<u4"), ("first_sample", "<u8"), ("last_sample", "<u8"),
+                        ("peak_sample", "<u8"), ("peak_trial", "<u4"), ("peak_env", "<f4"), ("peak_sigma", "<f4"),
+                        ("peak_snr", "<f4")])
+assert EVENT_DTYPE.itemsize == 48
 
 EXPORTS = (
     "lofar_plan_create", "lofar_plan_destroy", "lofar_plan_set_band", "lofar_plan_set_delays",
     "lofar_plan_set_trials", "lofar_plan_set_filter", "lofar_plan_set_input",
-    "lofar_plan_set_trigger", "lofar_plan_workspace_bytes", "lofar_plan_set_allocator",
+    "lofar_plan_set_trigger", "lofar_plan_set_sigma_mode", "lofar_cluster",
+    "lofar_plan_workspace_bytes", "lofar_plan_set_allocator",
     "lofar_plan_set_scratch_limit", "lofar_plan_chunking", "lofar_stream_state_bytes",
     "lofar_stream_get_state", "lofar_stream_set_state", "lofar_beamform_dedisperse",
     "lofar_inverse_ppf", "lofar_trigger", "lofar_run_block", "lofar_stream_reset",
@@ -64,6 +71,8 @@ def load() -> ctypes.CDLL:
         "lofar_plan_set_filter": (i, [vp, vp]),
         "lofar_plan_set_input": (i, [vp, i, i]),
         "lofar_plan_set_trigger": (i, [vp, d, i, u32]),
+        "lofar_plan_set_sigma_mode": (i, [vp, i, vp]),
+        "lofar_cluster": (i, [vp, vp, vp, u64, vp, vp, u32, vp]),
         "lofar_plan_workspace_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
         "lofar_plan_set_allocator": (i, [vp, vp, vp, vp]),
         "lofar_plan_set_scratch_limit": (i, [vp, c.c_size_t]),
@@ -177,6 +186,19 @@ class Plan:
         _check(self._lib.lofar_plan_set_trigger(self._h, float(kappa), env_window, max_candidates), "lofar_plan_set_trigger")
         self.max_candidates = max_candidates
 
+    def set_sigma_mode(self, mode: int, sigma_init=None):
+        if sigma_init is None:
+            _check(self._lib.lofar_plan_set_sigma_mode(self._h, mode, None), "lofar_plan_set_sigma_mode")
+        else:
+            si = np.ascontiguousarray(sigma_init, dtype=np.float32)
+            assert si.size == self.nseries
+            _check(self._lib.lofar_plan_set_sigma_mode(self._h, mode, si.ctypes.data), "lofar_plan_set_sigma_mode")
+
+    def cluster(self, cand, count, gap_samples: int, events, nevents, stream=None):
+        """events: device uint8 tensor [max_events][48]; nevents: device int32[1]."""
+        _check(self._lib.lofar_cluster(self._h, _ptr(cand), _ptr(count), int(gap_samples), _ptr(events), _ptr(nevents),
+                                       events.shape[0], _stream_ptr(stream)), "lofar_cluster")
+
     def workspace_bytes(self) -> int:
         n = ctypes.c_size_t()
         _check(self._lib.lofar_plan_workspace_bytes(self._h, ctypes.byref(n)), "lofar_plan_workspace_bytes")
@@ -286,6 +308,13 @@ def new_outputs(plan: Plan, slices: int, device="cuda"):
     count = torch.zeros(1, dtype=torch.int32, device=device)
     sigma = torch.zeros(plan.nseries, dtype=torch.float32, device=device)
     return series, cand, count, sigma
+
+
+def events_to_numpy(events, nevents) -> np.ndarray:
+    n = int(nevents.item()) if hasattr(nevents, "item") else int(nevents)
+    raw = events.cpu().numpy() if hasattr(events, "cpu") else np.asarray(events)
+    rec = raw.reshape(-1).view(EVENT_DTYPE)
+    return rec[:min(n, rec.size)].copy()
 
 
 def candidates_to_numpy(cand, count) -> np.ndarray:

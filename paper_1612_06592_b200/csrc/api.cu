@@ -75,6 +75,8 @@ void free_tables(lofar_plan *p)
     dev_free(p, p->dW); dev_free(p, p->dDph); dev_free(p, p->dGs); dev_free(p, p->dTw);
     dev_free(p, p->dHist[0]); dev_free(p, p->dHist[1]); dev_free(p, p->dTail);
     dev_free(p, p->dZ); dev_free(p, p->dPartial); dev_free(p, p->dChunkMax);
+    dev_free(p, p->dItems); dev_free(p, p->dNItems); dev_free(p, p->dSigmaRef); dev_free(p, p->dThr); dev_free(p, p->dHist0);
+    p->have_ref = false;
     free_staging(p);
     p->device_bytes = 0;
     p->built = false;
@@ -134,13 +136,14 @@ size_t sample_bytes(const lofar_plan *p) { return p->dtype == LOFAR_CI16 ? 4 : 2
 // these, lofar_plan_workspace_bytes reports their sum.
 struct Layout {
     bool tc;                 // tensor-core operand images wanted (int8 input)
-    size_t W, Dph, gs, tw, wimg, hist, tail, Z, partial, chunkmax;
+    size_t W, Dph, gs, tw, wimg, hist, tail, Z, partial, chunkmax, items;
     size_t x_bytes, cand, sigma;   // streaming staging (per slot)
     long long cap, zchunk, nsteps;
     size_t table_bytes() const
     {
         return (W + Dph + gs + tw + Z) * sizeof(float2) + wimg * sizeof(unsigned short) +
-               (2 * hist + tail + chunkmax) * sizeof(float) + partial * sizeof(double);
+               (3 * hist + tail + chunkmax + 2 * sigma) * sizeof(float) + partial * sizeof(double) +
+               items * sizeof(int2) + sizeof(uint32_t);
     }
     size_t staging_bytes() const
     {
@@ -166,9 +169,25 @@ Layout layout(const lofar_plan *p)
     L.nsteps = L.cap / kStepSlices;
     L.partial = ns * (size_t)L.nsteps;
     L.chunkmax = ns * (size_t)L.nsteps;
+    L.items = 16384;                   // flagged chunks per block before the scan falls back to all of them
     L.x_bytes = S * 2 * K * (size_t)(p->max_slices > 0 ? p->max_slices : 0) * sample_bytes(p);
     L.cand = p->max_cand; L.sigma = ns;
     return L;
+}
+
+// Causal sigma: the reference level a stream starts with (lofar_plan_set_sigma_mode).
+lofar_status load_sigma_init(lofar_plan *p, cudaStream_t st)
+{
+    p->have_ref = false;
+    const size_t ns = (size_t)p->B * p->D;
+    if (p->sigma_mode != LOFAR_SIGMA_CAUSAL || p->sigma_init.size() != ns) return LOFAR_OK;
+    p->thr_init.resize(ns);
+    for (size_t i = 0; i < ns; ++i) p->thr_init[i] = (float)p->kappa * p->sigma_init[i];
+    // the host vectors live in the plan, so the stream-ordered copies may read them later
+    CU(cudaMemcpyAsync(p->dSigmaRef, p->sigma_init.data(), ns * sizeof(float), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(p->dThr, p->thr_init.data(), ns * sizeof(float), cudaMemcpyHostToDevice, st));
+    p->have_ref = true;
+    return LOFAR_OK;
 }
 
 lofar_status build(lofar_plan *p)
@@ -246,6 +265,15 @@ lofar_status build(lofar_plan *p)
     p->chunkmax_pitch = L.nsteps;
     if ((st = dev_alloc(p, &p->dPartial, L.partial)) != LOFAR_OK) return st;
     if ((st = dev_alloc(p, &p->dChunkMax, L.chunkmax)) != LOFAR_OK) return st;
+    p->items_cap = (uint32_t)L.items;
+    if ((st = dev_alloc(p, &p->dItems, L.items)) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dNItems, 1)) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dSigmaRef, L.sigma)) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dThr, L.sigma)) != LOFAR_OK) return st;
+    if ((st = dev_alloc(p, &p->dHist0, L.hist)) != LOFAR_OK) return st;
+    CU(cudaMemset(p->dNItems, 0, sizeof(uint32_t)));
+    if ((st = load_sigma_init(p, nullptr)) != LOFAR_OK) return st;
+    CU(cudaDeviceSynchronize());       // build is the one place that may block: tables are in place when it returns
     p->built = true;
     return LOFAR_OK;
 }
@@ -259,7 +287,7 @@ lofar_status apply_reset(lofar_plan *p, cudaStream_t st)
     CU(cudaMemsetAsync(p->dHist[1], 0, hist, st));
     if (p->dTail) CU(cudaMemsetAsync(p->dTail, 0, (size_t)p->B * p->D * (p->env_window - 1) * sizeof(float), st));
     p->reset_pending = false;
-    return LOFAR_OK;
+    return load_sigma_init(p, st);
 }
 
 lofar_status ensure(lofar_plan *p, int slices)
@@ -298,11 +326,18 @@ int beamform_dispatch(lofar_plan *p, const BeamformArgs &b, cudaStream_t st)
     return launch_beamform(b, st);
 }
 
+struct EmitTo { lofar_candidate *cand; uint32_t *count; };   // cand == nullptr: no emission from the epilogue
+
 lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, int ztile, long long nc, int zmap_trials,
                      float *series, long long series_pitch, long long out0, int *partial0, long long step0,
-                     cudaStream_t st)
+                     cudaStream_t st, EmitTo em = EmitTo{nullptr, nullptr})
 {
     IppfArgs a{};
+    a.D = p->D; a.offset = p->offset;
+    if (em.cand) {
+        a.thr = p->dThr; a.sigma_ref = p->dSigmaRef;
+        a.cand = em.cand; a.count = em.count; a.cap = p->max_cand;
+    }
     a.Z = Z; a.zpitch = zpitch; a.ztile = ztile; a.nc = nc;
     a.series = series; a.series_pitch = series_pitch; a.out0 = out0;
     a.Dph = p->dDph; a.zmap_trials = zmap_trials;
@@ -335,6 +370,9 @@ TriggerArgs trigger_args(lofar_plan *p, const float *series, long long N, lofar_
     t.nchunks = (N + 16383) / 16384;
     t.sigma = sigma; t.cand = cand; t.count = count; t.cap = p->max_cand;
     t.offset = p->offset;
+    t.sigma_thr = (p->sigma_mode == LOFAR_SIGMA_CAUSAL && p->have_ref) ? p->dSigmaRef : sigma;
+    t.zero_count = 1;
+    t.items = p->dItems; t.nitems = p->dNItems; t.items_cap = p->items_cap;
     return t;
 }
 
@@ -350,6 +388,19 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
                             uint32_t *count, float *sigma, cudaStream_t st)
 {
     const long long T = slices, N = T * kMfft;
+    const int ns = p->B * p->D;
+    const bool causal = p->sigma_mode == LOFAR_SIGMA_CAUSAL;
+    // how the candidates of this block are found:
+    //   emit   -- threshold known before the block: decided in the inverse-PPF epilogue;
+    //   scan   -- two-pass: sigma of this block, then the stored series is re-read where its maximum allows;
+    //   rescan -- two-pass without a series: those places are recomputed from X.
+    const bool emit = causal && p->have_ref;
+    const bool rescan = !emit && series == nullptr;
+    if ((causal || series == nullptr) && p->env_window != 1) return LOFAR_E_INVALID;
+    if (emit || rescan) CU(cudaMemsetAsync(count, 0, sizeof(uint32_t), st));
+    if (rescan)
+        CU(cudaMemcpyAsync(p->dHist0, p->dHist[p->hist_parity], (size_t)ns * (kTaps - 1) * kMfft * sizeof(float),
+                           cudaMemcpyDeviceToDevice, st));
     int partial0 = 0;
     for (long long c0 = 0; c0 < T; c0 += p->zchunk) {
         const long long nc = (T - c0 < p->zchunk) ? T - c0 : p->zchunk;
@@ -365,10 +416,11 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
             p->launches += n;
         }
         lofar_status s = do_ippf(p, p->dZ, p->zchunk, 1, nc, p->D > 1 ? p->D : 0, series, N, c0 * kMfft, &partial0,
-                                 c0 / kStepSlices, st);
+                                 c0 / kStepSlices, st, emit ? EmitTo{cand, count} : EmitTo{nullptr, nullptr});
         if (s != LOFAR_OK) return s;
     }
     TriggerArgs t = trigger_args(p, series, N, cand, count, sigma);
+    t.zero_count = (emit || rescan) ? 0 : 1;
     int n;
     ProfScope prof(p, 2, st);
     if (p->env_window == 1) {
@@ -378,11 +430,37 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
         if ((n = launch_trigger_reduce(t, st)) < 0) return LOFAR_E_CUDA;
         p->launches += n;
     }
-    if ((n = launch_trigger_finish(t, st)) < 0) return LOFAR_E_CUDA;
+    if ((n = launch_trigger_sigma(t, st)) < 0) return LOFAR_E_CUDA;
+    p->launches += n;
+    if (!emit) {
+        if ((n = launch_trigger_flag(t, st)) < 0) return LOFAR_E_CUDA;
+        p->launches += n;
+        if (rescan) {
+            RescanArgs r{};
+            r.X = X; r.xpitch = T; r.dtype = p->dtype; r.T = T;
+            r.W = p->dW; r.Dph = p->dDph; r.S = p->S; r.K = p->K; r.k0 = p->k0; r.B = p->B; r.D = p->D;
+            r.hist0 = p->dHist0; r.gs = p->dGs; r.tw = p->dTw;
+            r.items = p->dItems; r.nitems = p->dNItems; r.items_cap = p->items_cap;
+            r.sigma = sigma; r.kappa = (float)p->kappa;
+            r.chunkmax = p->dChunkMax; r.chunkmax_pitch = p->chunkmax_pitch;
+            r.cand = cand; r.count = count; r.cap = p->max_cand; r.offset = p->offset;
+            if ((n = launch_rescan(r, p->num_sms, st)) < 0) return LOFAR_E_CUDA;
+        } else {
+            if ((n = launch_trigger_scan(t, 4 * p->num_sms, st)) < 0) return LOFAR_E_CUDA;
+        }
+        p->launches += n;
+    }
+    if ((n = launch_trigger_sort(t, (emit || rescan) && p->D > 1, st)) < 0) return LOFAR_E_CUDA;
     p->launches += n;
     if (p->env_window > 1) {
-        if ((n = launch_tail_save(series, N, N, p->B * p->D, p->env_window, p->dTail, st)) < 0) return LOFAR_E_CUDA;
+        if ((n = launch_tail_save(series, N, N, ns, p->env_window, p->dTail, st)) < 0) return LOFAR_E_CUDA;
         p->launches += n;
+    }
+    if (causal) {
+        // this block's sigma is the level the next block is measured against
+        if ((n = launch_sigma_ref(sigma, (float)p->kappa, ns, p->dSigmaRef, p->dThr, st)) < 0) return LOFAR_E_CUDA;
+        p->launches += n;
+        p->have_ref = true;
     }
     p->offset += (uint64_t)N;
     return LOFAR_OK;
@@ -498,6 +576,27 @@ lofar_status lofar_plan_set_allocator(lofar_plan *p, void *(*alloc)(size_t, void
     return LOFAR_OK;
 }
 
+lofar_status lofar_plan_set_sigma_mode(lofar_plan *p, lofar_sigma_mode mode, const float *sigma_init)
+{
+    if (!p || (mode != LOFAR_SIGMA_BLOCK && mode != LOFAR_SIGMA_CAUSAL)) return LOFAR_E_INVALID;
+    p->sigma_mode = mode;
+    if (sigma_init && mode == LOFAR_SIGMA_CAUSAL) p->sigma_init.assign(sigma_init, sigma_init + (size_t)p->B * p->D);
+    else p->sigma_init.clear();
+    p->built = false;
+    return LOFAR_OK;
+}
+
+lofar_status lofar_cluster(lofar_plan *p, const lofar_candidate *cand, const uint32_t *count, uint64_t gap,
+                           lofar_event *events, uint32_t *nevents, uint32_t max_events, void *stream)
+{
+    if (!p || !cand || !count || !events || !nevents || max_events == 0) return LOFAR_E_INVALID;
+    const int n = launch_cluster(cand, count, p->max_cand, p->D, gap, events, nevents, max_events,
+                                 static_cast<cudaStream_t>(stream));
+    if (n < 0) return LOFAR_E_CUDA;
+    p->launches += n;
+    return LOFAR_OK;
+}
+
 lofar_status lofar_plan_set_scratch_limit(lofar_plan *p, size_t bytes)
 {
     if (!p || bytes == 0) return LOFAR_E_INVALID;
@@ -565,17 +664,30 @@ lofar_status lofar_trigger(lofar_plan *p, const float *series, int slices, lofar
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if ((s = apply_reset(p, st)) != LOFAR_OK) return s;
     const long long N = (long long)slices * kMfft;
+    const bool causal = p->sigma_mode == LOFAR_SIGMA_CAUSAL;
+    if (causal && p->env_window != 1) return LOFAR_E_INVALID;
     TriggerArgs t = trigger_args(p, series, N, cand, count, sigma);
     t.nparts = (int)t.nchunks;
     int n;
     ProfScope prof(p, 2, st);
     if ((n = launch_trigger_reduce(t, st)) < 0) return LOFAR_E_CUDA;
     p->launches += n;
-    if ((n = launch_trigger_finish(t, st)) < 0) return LOFAR_E_CUDA;
+    if ((n = launch_trigger_sigma(t, st)) < 0) return LOFAR_E_CUDA;
+    p->launches += n;
+    if ((n = launch_trigger_flag(t, st)) < 0) return LOFAR_E_CUDA;
+    p->launches += n;
+    if ((n = launch_trigger_scan(t, 4 * p->num_sms, st)) < 0) return LOFAR_E_CUDA;
+    p->launches += n;
+    if ((n = launch_trigger_sort(t, false, st)) < 0) return LOFAR_E_CUDA;
     p->launches += n;
     if (p->env_window > 1) {
         if ((n = launch_tail_save(series, N, N, p->B * p->D, p->env_window, p->dTail, st)) < 0) return LOFAR_E_CUDA;
         p->launches += n;
+    }
+    if (causal) {
+        if ((n = launch_sigma_ref(sigma, (float)p->kappa, p->B * p->D, p->dSigmaRef, p->dThr, st)) < 0) return LOFAR_E_CUDA;
+        p->launches += n;
+        p->have_ref = true;
     }
     p->offset += (uint64_t)N;
     return LOFAR_OK;
@@ -586,7 +698,7 @@ lofar_status lofar_run_block(lofar_plan *p, const void *X, int slices, float *se
 {
     lofar_status s = ensure(p, slices);
     if (s != LOFAR_OK) return s;
-    if (!series || !cand || !count || !sigma) return LOFAR_E_INVALID;
+    if (!cand || !count || !sigma) return LOFAR_E_INVALID;      // series == NULL: trigger-only
     if ((s = check_x(p, X, slices)) != LOFAR_OK) return s;
     if ((s = apply_reset(p, static_cast<cudaStream_t>(stream))) != LOFAR_OK) return s;
     return run_block_impl(p, X, slices, series, cand, count, sigma, static_cast<cudaStream_t>(stream));
@@ -609,7 +721,7 @@ lofar_status lofar_stream_push(lofar_plan *p, const void *X_host, int slices, fl
 {
     lofar_status s = ensure(p, slices);
     if (s != LOFAR_OK) return s;
-    if (!X_host || !series) return LOFAR_E_INVALID;
+    if (!X_host) return LOFAR_E_INVALID;                        // series == NULL: trigger-only
     if (((size_t)slices * sample_bytes(p)) & 15) return LOFAR_E_ALIGN;
     if (p->pushes >= kCountRing) return LOFAR_E_STATE;   // call lofar_stream_sync at least every 64 pushes
     const int ns = p->B * p->D;
@@ -676,7 +788,8 @@ constexpr uint32_t kStateMagic = 0x4c4f4631u;   // "LOF1"
 size_t state_bytes(const lofar_plan *p)
 {
     const size_t ns = (size_t)p->B * p->D;
-    return sizeof(StateHeader) + ns * (kTaps - 1) * kMfft * sizeof(float) + ns * (size_t)(p->env_window - 1) * sizeof(float);
+    return sizeof(StateHeader) + ns * (kTaps - 1) * kMfft * sizeof(float) + ns * (size_t)(p->env_window - 1) * sizeof(float) +
+           ns * sizeof(float);                 // + the causal reference level (header.reserved = 1 if valid)
 }
 }  // namespace
 
@@ -699,15 +812,15 @@ lofar_status lofar_stream_get_state(lofar_plan *p, void *state_host, size_t byte
     quiesce(p);
     const size_t ns = (size_t)p->B * p->D, hist = ns * (kTaps - 1) * kMfft * sizeof(float);
     const size_t tail = ns * (size_t)(p->env_window - 1) * sizeof(float);
-    StateHeader h{kStateMagic, (uint32_t)ns, (uint32_t)kTaps, (uint32_t)kMfft, (uint32_t)p->env_window, 0u, p->offset};
+    StateHeader h{kStateMagic, (uint32_t)ns, (uint32_t)kTaps, (uint32_t)kMfft, (uint32_t)p->env_window,
+                  (p->have_ref && !p->reset_pending) ? 1u : 0u, p->offset};
     char *dst = static_cast<char *>(state_host);
     std::memcpy(dst, &h, sizeof(h));
-    if (p->reset_pending) {
-        std::memset(dst + sizeof(h), 0, hist + tail);
-        return LOFAR_OK;
-    }
+    std::memset(dst + sizeof(h), 0, hist + tail + ns * sizeof(float));
+    if (p->reset_pending) return LOFAR_OK;
     CU(cudaMemcpy(dst + sizeof(h), p->dHist[p->hist_parity], hist, cudaMemcpyDeviceToHost));
     if (tail) CU(cudaMemcpy(dst + sizeof(h) + hist, p->dTail, tail, cudaMemcpyDeviceToHost));
+    if (h.reserved) CU(cudaMemcpy(dst + sizeof(h) + hist + tail, p->dSigmaRef, ns * sizeof(float), cudaMemcpyDeviceToHost));
     return LOFAR_OK;
 }
 
@@ -731,6 +844,15 @@ lofar_status lofar_stream_set_state(lofar_plan *p, const void *state_host, size_
     const char *src = static_cast<const char *>(state_host);
     CU(cudaMemcpy(p->dHist[p->hist_parity], src + sizeof(h), hist, cudaMemcpyHostToDevice));
     if (tail) CU(cudaMemcpy(p->dTail, src + sizeof(h) + hist, tail, cudaMemcpyHostToDevice));
+    p->have_ref = false;
+    if (h.reserved && p->sigma_mode == LOFAR_SIGMA_CAUSAL) {
+        std::vector<float> ref(ns), thr(ns);
+        std::memcpy(ref.data(), src + sizeof(h) + hist + tail, ns * sizeof(float));
+        for (size_t i = 0; i < ns; ++i) thr[i] = (float)p->kappa * ref[i];
+        CU(cudaMemcpy(p->dSigmaRef, ref.data(), ns * sizeof(float), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(p->dThr, thr.data(), ns * sizeof(float), cudaMemcpyHostToDevice));
+        p->have_ref = true;
+    }
     p->offset = h.offset;
     p->reset_pending = false;
     return LOFAR_OK;

@@ -259,11 +259,38 @@ __device__ __forceinline__ void fft512_warp(float2 *row, const float2 *stw, int 
     __syncwarp();
 }
 
+// Where candidates found in the FIR epilogue go (threshold known before the block: causal sigma, or the rescan).
+struct Emit {
+    lofar_candidate *cand;
+    uint32_t *count;
+    uint32_t cap;
+    uint32_t series, trial;
+    float thr, sigma;        // thr = kappa * sigma; +inf disables emission
+    uint64_t sample0;        // global index of sample 0 of the series slice the step starts at
+};
+
+// Rare path: one record per sample above the threshold (all trials; the best trial is selected after the sort).
+__device__ __noinline__ void emit_pair(const Emit &e, uint64_t n, float vx, float vy)
+{
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        const float v = fabsf(c ? vy : vx);
+        if (v > e.thr) {
+            const uint32_t slot = atomicAdd(e.count, 1u);
+            if (slot < e.cap) {
+                lofar_candidate r;
+                r.series = e.series; r.trial = e.trial; r.sample = n + c; r.env = v; r.sigma = e.sigma;
+                e.cand[slot] = r;
+            }
+        }
+    }
+}
+
 // Synthesis FIR of one step: out[j] = sum_t g[t] * win[15 + j - t], j = 0..15, window = prev rows 1..15 + cur rows
 // 0..15, column pn; FULL = all 16 output slices valid (no predicates on the fast path).
 template <bool FULL>
 __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, const u64 (&g)[kP], int pn, float *out,
-                                         int tid, int nvalid, u64 &ssum2, float &smax)
+                                         int tid, int nvalid, const Emit &em, u64 &ssum2, float &smax)
 {
     u64 acc[kStep];
 #pragma unroll
@@ -284,7 +311,9 @@ __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, 
                 const float vx = LO(acc[j]), vy = HI(acc[j]);
                 if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)j * kM + 2 * tid), make_float2(vx, vy));
                 ssum2 = fma2(acc[j], acc[j], ssum2);
-                smax = fmaxf(smax, fmaxf(fabsf(vx), fabsf(vy)));
+                const float m = fmaxf(fabsf(vx), fabsf(vy));
+                smax = fmaxf(smax, m);
+                if (m > em.thr) emit_pair(em, em.sample0 + (uint64_t)j * kM + 2 * tid, vx, vy);
             }
         }
     }
@@ -340,7 +369,13 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     bool async = stage_fill(c, q_first, stage, bar, tid);
 
     float *out = a.series ? a.series + (size_t)series * a.series_pitch + a.out0 : nullptr;
+    float *yout = a.yout ? a.yout + (size_t)series * a.yout_pitch + a.out0 : nullptr;
     double dsum = 0.0;
+    Emit em;
+    em.cand = a.cand; em.count = a.count; em.cap = a.cap;
+    em.series = (uint32_t)series; em.trial = (uint32_t)(series % a.D);
+    em.thr = a.thr ? a.thr[series] : __int_as_float(0x7f800000);
+    em.sigma = a.thr ? a.sigma_ref[series] : 0.f;
 
     for (long long q = q_first; q < qe; q += kStep) {
         if (async) { while (!mbar_try_wait(bar, phase)) {} phase ^= 1; }
@@ -351,13 +386,28 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
         fft512_warp(cur + warp * kRow, stw, lane);
         __syncthreads();
 
-        if (q >= qs) {
+        if (q >= qs && yout) {
+            // LSMR inversion (f1): hand the inverse-DFT rows to the solver instead of applying the matched FIR
+            const int nvalid = (qe - q < kStep) ? (int)(qe - q) : kStep;
+            for (int j = 0; j < nvalid; ++j)
+                *reinterpret_cast<float2 *>(yout + (size_t)(q + j) * kM + 2 * tid) = cur[j * kRow + pn];
+            if (is_last && q + kStep >= qe) {
+                float *h = a.hist_out + (size_t)series * (kP - 1) * kM;
+                for (int idx = 0; idx < kP - 1; ++idx) {
+                    const int i = nvalid - (kP - 1) + idx;
+                    const float2 v = (i < 0) ? prev[(kStep + i) * kRow + pn] : cur[i * kRow + pn];
+                    *reinterpret_cast<float2 *>(h + (size_t)idx * kM + 2 * tid) = v;
+                }
+            }
+            __syncthreads();
+        } else if (q >= qs) {
             const int nvalid = (qe - q < kStep) ? (int)(qe - q) : kStep;
             u64 ssum2 = 0ull;
             float smax = 0.f;
             float *o = out ? out + (size_t)q * kM : nullptr;
-            if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
-            else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
+            em.sample0 = a.offset + (uint64_t)a.out0 + (uint64_t)q * kM;
+            if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, em, ssum2, smax);
+            else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, em, ssum2, smax);
             dsum += (double)(LO(ssum2) + HI(ssum2));
 #pragma unroll
             for (int s = 16; s > 0; s >>= 1) smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, s));
@@ -395,11 +445,105 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     }
 }
 
+
+// ---- series-free two-pass trigger: recompute the flagged steps from X ------------------------------
+__device__ __forceinline__ float2 read_cx(const void *X, int dtype, size_t idx)
+{
+    if (dtype == LOFAR_CI16) {
+        const short2 v = reinterpret_cast<const short2 *>(X)[idx];
+        return make_float2((float)v.x, (float)v.y);
+    }
+    const char2 v = reinterpret_cast<const char2 *>(X)[idx];
+    return make_float2((float)v.x, (float)v.y);
+}
+
+// Beam sums of one beam for the 16 slices starting at q, straight into the stage (plain fp32 sums).
+__device__ __forceinline__ void stage_from_x(const RescanArgs &r, int beam, long long q, float2 *stage, int tid)
+{
+    for (int idx = tid; idx < r.K * kStep; idx += kThreads) {
+        const int j = idx >> 4, t = idx & 15;
+        float2 acc = make_float2(0.f, 0.f);
+        if (q + t < r.T) {
+            const float2 *w = r.W + ((size_t)j * r.B + beam) * r.S;
+            for (int s = 0; s < r.S; ++s) {
+                const size_t i0 = ((size_t)(2 * s) * r.K + j) * (size_t)r.xpitch + (size_t)(q + t);
+                const float2 x0 = read_cx(r.X, r.dtype, i0), x1 = read_cx(r.X, r.dtype, i0 + (size_t)r.K * r.xpitch);
+                const float xr = x0.x + x1.x, xi = x0.y + x1.y;
+                const float2 ww = __ldg(w + s);
+                acc.x = fmaf(ww.x, xr, fmaf(-ww.y, xi, acc.x));
+                acc.y = fmaf(ww.x, xi, fmaf(ww.y, xr, acc.y));
+            }
+        }
+        stage[idx] = acc;
+    }
+}
+
+__global__ void __launch_bounds__(kThreads, 1) rescan_kernel(RescanArgs r)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float2 *stage = reinterpret_cast<float2 *>(smem_raw);
+    float2 *buf0 = stage + kStageF2;
+    float2 *buf1 = buf0 + kStep * kRow;
+    float2 *stw = buf1 + kStep * kRow;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t total = *r.nitems < r.items_cap ? *r.nitems : r.items_cap;
+    if (blockIdx.x >= total) return;
+    for (int i = tid; i < kTwCount; i += kThreads) stw[i] = r.tw[i];
+    u64 g[kP];
+#pragma unroll
+    for (int t = 0; t < kP; ++t) { const float2 v = __ldg(r.gs + t * kH + tid); g[t] = PK(v.x, v.y); }
+    const int pn = pad(tid);
+    __syncthreads();
+
+    for (uint32_t it = blockIdx.x; it < total; it += gridDim.x) {
+        const int beam = r.items[it].x;
+        const long long q = (long long)r.items[it].y * kStep;
+        for (int d = 0; d < r.D; ++d) {
+            const int series = beam * r.D + d;
+            const float sig = r.sigma[series], thr = r.kappa * sig;
+            if (r.chunkmax[(size_t)series * r.chunkmax_pitch + r.items[it].y] < thr * 0.99999f) continue;
+            Ctx c;
+            c.Zs = nullptr; c.ph = r.D > 1 ? r.Dph + (size_t)d * r.K : nullptr;
+            c.zpitch = 0; c.nc = r.T; c.K = r.K; c.k0 = r.k0; c.bulk_rows = 0; c.tiled = 0;
+            if (q == 0) {
+                const float *h = r.hist0 + (size_t)series * (kP - 1) * kM;
+#pragma unroll
+                for (int i = 0; i < kP - 1; ++i)
+                    buf0[(i + 1) * kRow + pn] = *reinterpret_cast<const float2 *>(h + (size_t)i * kM + 2 * tid);
+            } else {
+                stage_from_x(r, beam, q - kStep, stage, tid);
+                __syncthreads();
+                prepass(c, stage, buf0, stw, tid);
+                __syncthreads();
+                fft512_warp(buf0 + warp * kRow, stw, lane);
+            }
+            __syncthreads();
+            stage_from_x(r, beam, q, stage, tid);
+            __syncthreads();
+            prepass(c, stage, buf1, stw, tid);
+            __syncthreads();
+            fft512_warp(buf1 + warp * kRow, stw, lane);
+            __syncthreads();
+            Emit em;
+            em.cand = r.cand; em.count = r.count; em.cap = r.cap;
+            em.series = (uint32_t)series; em.trial = (uint32_t)d; em.thr = thr; em.sigma = sig;
+            em.sample0 = r.offset + (uint64_t)q * kM;
+            const int nvalid = (r.T - q < kStep) ? (int)(r.T - q) : kStep;
+            u64 ssum2 = 0ull;
+            float smax = 0.f;
+            fir_step<false>(buf0, buf1, g, pn, nullptr, tid, nvalid, em, ssum2, smax);
+            __syncthreads();
+        }
+    }
+}
+
 }  // namespace
 
 int ippf_configure()
 {
     cudaError_t e = cudaFuncSetAttribute(ippf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(rescan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
     return e == cudaSuccess ? 0 : -1;
 }
 
@@ -408,6 +552,12 @@ int launch_ippf(const IppfArgs &a, cudaStream_t st)
     if (a.nc <= 0) return 0;
     dim3 grid((unsigned)(a.nseries * a.nspans));
     ippf_kernel<<<grid, kThreads, kSmemBytes, st>>>(a);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
+
+int launch_rescan(const RescanArgs &a, int grid, cudaStream_t st)
+{
+    rescan_kernel<<<grid, kThreads, kSmemBytes, st>>>(a);
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 

@@ -46,6 +46,36 @@ struct IppfArgs {
     float *chunkmax;      // [nseries][chunkmax_pitch] max |xhat| per 16-slice step
     long long chunkmax_pitch, step0;
     int vec_ok;           // Z rows are 16-byte aligned at every step start (128-byte bulk copies allowed)
+    // threshold known before the block (causal sigma): candidates are emitted from the FIR epilogue
+    const float *thr;     // [nseries] kappa * sigma_ref, or nullptr
+    const float *sigma_ref;
+    lofar_candidate *cand;
+    uint32_t *count;
+    uint32_t cap;
+    int D;                // trials per beam (candidate.trial = series % D)
+    uint64_t offset;      // stream offset of sample 0 of the block
+    float *yout;          // nullptr, or [nseries][yout_pitch] float: the inverse-DFT rows y[q][1024] (LSMR inversion, f1);
+    long long yout_pitch; //   the FIR is skipped and no series is written
+};
+
+// Series-free two-pass trigger (series == NULL, sigma of this block): the flagged (beam, 16-slice step) items are
+// recomputed from X -- SIMT beam sums, transform, FIR -- and compared with kappa * sigma.
+struct RescanArgs {
+    const void *X; long long xpitch; int dtype;      // [S][2][K][xpitch] complex ints, T = slices of the block
+    long long T;
+    const float2 *W;      // [K][B][S]
+    const float2 *Dph;    // [D][K] (applied when D > 1)
+    int S, K, k0, B, D;
+    const float *hist0;   // [nseries][15][1024] history at the start of the block
+    const float2 *gs, *tw;
+    const int2 *items;    // (beam, step) list
+    const uint32_t *nitems;
+    uint32_t items_cap;
+    const float *sigma;   // [nseries] of this block
+    float kappa;
+    const float *chunkmax; long long chunkmax_pitch;
+    lofar_candidate *cand; uint32_t *count; uint32_t cap;
+    uint64_t offset;
 };
 
 struct TriggerArgs {
@@ -64,7 +94,13 @@ struct TriggerArgs {
     uint32_t *count;
     uint32_t cap;
     uint64_t offset;      // stream offset of sample 0 of this block
+    const float *sigma_thr;   // [nseries] level the candidates are measured against (= sigma, or the previous block's)
+    int zero_count;       // sigma_kernel resets *count (not when candidates were emitted by the inverse PPF)
+    int2 *items;          // flagged (beam, 16384-sample chunk) list and its length
+    uint32_t *nitems;
+    uint32_t items_cap;
 };
+
 
 // kernel launchers (each returns the number of kernels it launched, or -1 on a launch error)
 int launch_beamform(const BeamformArgs &a, cudaStream_t st);
@@ -76,8 +112,15 @@ void tc_build_image(const double *w_re, const double *w_im, int S, int B, unsign
 int launch_beamform_tc(const BeamformArgs &a, const void *wimg, cudaStream_t st);
 int tc_configure();                                     // opt in to the large dynamic shared memory (current device)
 int ippf_configure();                                   // opt in to the large dynamic shared memory
+int launch_rescan(const RescanArgs &a, int grid, cudaStream_t st);
 int launch_trigger_reduce(const TriggerArgs &a, cudaStream_t st);   // sum e^2 + chunk max from the series
-int launch_trigger_finish(const TriggerArgs &a, cudaStream_t st);   // sigma, threshold scan, sort
+int launch_trigger_sigma(const TriggerArgs &a, cudaStream_t st);    // sigma from the partial sums
+int launch_trigger_flag(const TriggerArgs &a, cudaStream_t st);     // list of chunks whose maximum can reach the threshold
+int launch_trigger_scan(const TriggerArgs &a, int grid, cudaStream_t st);   // threshold scan of the flagged chunks
+int launch_trigger_sort(const TriggerArgs &a, bool unique, cudaStream_t st);   // order (and best-trial dedupe)
+int launch_sigma_ref(const float *sigma, float kappa, int nseries, float *sigma_ref, float *thr, cudaStream_t st);
+int launch_cluster(const lofar_candidate *cand, const uint32_t *count, uint32_t cap, int D, uint64_t gap,
+                   lofar_event *events, uint32_t *nevents, uint32_t max_events, cudaStream_t st);
 int launch_tail_save(const float *series, long long pitch, long long N, int nseries, int W,
                      float *tail, cudaStream_t st);
 
@@ -93,6 +136,8 @@ struct lofar_plan {
     double kappa = 6.0;
     int env_window = 1;
     uint32_t max_cand = 65536;
+    int sigma_mode = LOFAR_SIGMA_BLOCK;        // f3: LOFAR_SIGMA_CAUSAL judges block i against sigma of block i-1
+    std::vector<float> sigma_init, thr_init;   // optional reference level of the first block of a stream (and kappa times it)
     // device memory: every plan-owned device buffer goes through these (lofar_plan_set_allocator)
     void *(*alloc_fn)(size_t, void *) = nullptr;
     void (*free_fn)(void *, void *) = nullptr;
@@ -114,6 +159,12 @@ struct lofar_plan {
     int partial_pitch = 0;
     float *dChunkMax = nullptr;
     long long chunkmax_pitch = 0;
+    int2 *dItems = nullptr;            // flagged (beam, chunk) list of the trigger
+    uint32_t *dNItems = nullptr;
+    uint32_t items_cap = 0;
+    float *dSigmaRef = nullptr, *dThr = nullptr;   // causal sigma: level of the previous block and kappa times it
+    bool have_ref = false;
+    float *dHist0 = nullptr;           // history at the start of the block (series-free two-pass trigger)
     size_t device_bytes = 0;
     uint64_t offset = 0;
     uint64_t launches = 0;

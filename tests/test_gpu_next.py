@@ -1,0 +1,194 @@
+"""GPU parity for the rows "next" of SURVEY.md 8(f), each against the oracle function pinned in
+tests/test_oracle_next_pins.py: f3 (trigger-only mode, causal sigma, event clustering), f1 (LSMR inversion),
+f2 (exact de-dispersion), f4 (two-stage beamforming)."""
+import numpy as np
+import pytest
+
+from paper_1612_06592_b200 import binding, synth
+from parity_util import GUARD, assert_close, check_candidates, oracle_snr
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    binding.load()
+    return t
+
+
+def _blocks(w):
+    _, _, tau = synth.geometry(w)
+    return tau, [synth.generate_block(w, b, tau=tau) for b in range(w.blocks)]
+
+
+def _run(torch, p, X, T, want_series=True):
+    series, cand, count, sigma = binding.new_outputs(p, T)
+    p.run_block(torch.from_numpy(X).cuda(), T, series if want_series else None, cand, count, sigma)
+    torch.cuda.synchronize()
+    return (series.cpu().numpy() if want_series else None, binding.candidates_to_numpy(cand, count),
+            int(count.item()), sigma.cpu().numpy(), cand, count)
+
+
+# ------------------------------------------------------------------------------------------ f3
+TRIGGER_ONLY_CASES = [
+    dict(S=4, B=3, K=24, k0=200, T=208, dtype="ci8", n_pulses=5, blocks=2, kappa=4.5),
+    dict(S=4, B=2, K=16, k0=300, T=104, dtype="ci16", n_pulses=3, blocks=2, kappa=4.0),
+    dict(S=6, B=3, K=33, k0=470, T=72, dtype="ci8", stec=(8.0, 10.0, 12.0, 14.0), n_pulses=3, blocks=2, kappa=4.0),
+    dict(S=24, B=24, K=40, k0=100, T=136, dtype="ci8", n_pulses=4, blocks=2, kappa=4.5),
+]
+
+
+@pytest.mark.parametrize("kw", TRIGGER_ONLY_CASES)
+def test_trigger_only_mode_equals_the_oracle(torch, oracle, kw):
+    """series == NULL: no series in HBM, sigma and candidates as defined by O7/O8 -- the flagged
+    chunks are recomputed from X after sigma is known.  Two blocks (carried history at a flagged first step),
+    several scratch chunks, D = 1 and D > 1 (best trial per sample)."""
+    w = synth.small(**kw)
+    tau, blocks = _blocks(w)
+    pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa)
+    p = binding.plan_for(w, tau)
+    p.set_trigger(w.kappa, 1, 1 << 16)
+    p.set_scratch_limit(w.B * w.K * 8 * 64)           # three or four chunks per block
+    full = binding.plan_for(w, tau)
+    full.set_trigger(w.kappa, 1, 1 << 16)
+    offset = 0
+    for X in blocks:
+        ref, sig_ref, _, _ = pipe.run_block(X)
+        _, rec, n, sigma, _, _ = _run(torch, p, X, w.T, want_series=False)
+        np.testing.assert_allclose(sigma, sig_ref, rtol=5e-6)
+        env, sig = oracle_snr(oracle, ref, 1)
+        ndef, _ = check_candidates(rec, n, env, sig, w.B, w.D, w.kappa, offset)
+        assert ndef > 0
+        # and the list is the one the series path reports (up to the guard band)
+        _, rec_f, n_f, _, _, _ = _run(torch, full, X, w.T)
+        a = {(int(r["series"]) // w.D, int(r["sample"])) for r in rec}
+        b = {(int(r["series"]) // w.D, int(r["sample"])) for r in rec_f}
+        for bm, smp in a ^ b:
+            e = (env[bm * w.D:(bm + 1) * w.D, smp - offset] / sig[bm * w.D:(bm + 1) * w.D]).max() / w.kappa
+            assert abs(e - 1.0) <= GUARD
+        offset += w.T * 1024
+    p.destroy()
+    full.destroy()
+
+
+@pytest.mark.parametrize("with_series", [True, False])
+@pytest.mark.parametrize("kw", [
+    dict(S=4, B=3, K=24, k0=200, T=96, dtype="ci8", n_pulses=6, blocks=4, kappa=4.5),
+    dict(S=6, B=2, K=33, k0=470, T=72, dtype="ci8", stec=(8.0, 10.0, 12.0), n_pulses=4, blocks=3, kappa=4.0),
+])
+def test_causal_sigma_parity(torch, oracle, kw, with_series):
+    """LOFAR_SIGMA_CAUSAL: block i against sigma of block i-1 (O9); block 0 against itself.  Candidates come out of
+    the inverse-PPF epilogue (from block 1 on), with and without a series in HBM."""
+    w = synth.small(**kw)
+    tau, blocks = _blocks(w)
+    pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa, sigma_mode="causal")
+    p = binding.plan_for(w, tau)
+    p.set_trigger(w.kappa, 1, 1 << 16)
+    p.set_sigma_mode(binding.LOFAR_SIGMA_CAUSAL)
+    offset = 0
+    for i, X in enumerate(blocks):
+        ref, sig_ref, _, _ = pipe.run_block(X)
+        got, rec, n, sigma, _, _ = _run(torch, p, X, w.T, want_series=with_series)
+        np.testing.assert_allclose(sigma, sig_ref, rtol=5e-6)
+        if with_series:
+            for s in range(w.nseries):
+                assert_close(got[s], ref[s], f"block {i} series {s}")
+        env, _ = oracle_snr(oracle, ref, 1)
+        check_candidates(rec, n, env, pipe.last_sigma_ref, w.B, w.D, w.kappa, offset)
+        offset += w.T * 1024
+    # checkpoint in the middle of the stream: the reference level travels with the state
+    q = binding.plan_for(w, tau)
+    q.set_trigger(w.kappa, 1, 1 << 16)
+    q.set_sigma_mode(binding.LOFAR_SIGMA_CAUSAL)
+    q.set_state(p.get_state())
+    X = synth.generate_block(w, w.blocks, tau=tau)
+    _, rec_p, n_p, _, _, _ = _run(torch, p, X, w.T, want_series=with_series)
+    _, rec_q, n_q, _, _, _ = _run(torch, q, X, w.T, want_series=with_series)
+    assert n_p == n_q and np.array_equal(rec_p, rec_q)
+    p.destroy()
+    q.destroy()
+
+
+def test_causal_sigma_init_and_streaming(torch, oracle):
+    """sigma_init_host gives block 0 its level; the same through lofar_stream_push without a series."""
+    w = synth.small(S=4, B=3, K=24, k0=200, T=64, dtype="ci8", n_pulses=4, blocks=3, kappa=4.5)
+    tau, blocks = _blocks(w)
+    init = np.full(w.nseries, 1.05 * np.sqrt(0.9341 * 4 * w.K * 2 * w.S) * w.sigma_in)
+    pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa, sigma_mode="causal",
+                                 sigma_init=init)
+    p = binding.plan_for(w, tau)
+    p.set_trigger(w.kappa, 1, 8192)
+    p.set_sigma_mode(binding.LOFAR_SIGMA_CAUSAL, init)
+    p.stream_reset()
+    outs = []
+    for X in blocks:
+        cand_h = torch.zeros((8192, 24), dtype=torch.uint8).pin_memory()
+        count_h = torch.zeros(1, dtype=torch.int32).pin_memory()
+        sigma_h = torch.zeros(w.nseries, dtype=torch.float32).pin_memory()
+        Xh = torch.from_numpy(X).pin_memory()
+        p.stream_push(Xh, w.T, None, cand_h, count_h, sigma_h)
+        outs.append((Xh, cand_h, count_h, sigma_h))
+    p.stream_sync()
+    offset = 0
+    for X, (_, cand_h, count_h, sigma_h) in zip(blocks, outs):
+        ref, sig_ref, _, _ = pipe.run_block(X)
+        np.testing.assert_allclose(sigma_h.numpy(), sig_ref, rtol=5e-6)
+        env, _ = oracle_snr(oracle, ref, 1)
+        rec = binding.candidates_to_numpy(cand_h.numpy(), int(count_h.item()))
+        check_candidates(rec, int(count_h.item()), env, np.asarray(pipe.last_sigma_ref, dtype=np.float64), w.B, w.D,
+                         w.kappa, offset)
+        offset += w.T * 1024
+    p.destroy()
+
+
+def test_cluster_parity(torch, oracle):
+    """lofar_cluster on the candidate list of a block with pulses (several candidates per pulse) and on a hand-built
+    list, against O10."""
+    w = synth.small(S=6, B=4, K=33, k0=470, T=96, dtype="ci8", stec=(8.0, 10.0, 12.0), n_pulses=6, kappa=3.6)
+    tau, blocks = _blocks(w)
+    p = binding.plan_for(w, tau)
+    p.set_trigger(w.kappa, 1, 1 << 16)
+    _, rec, n, sigma, cand, count = _run(torch, p, blocks[0], w.T)
+    assert n > 50
+    for gap in (0, 3, 64, 5000):
+        events = torch.zeros((4096, 48), dtype=torch.uint8, device="cuda")
+        nev = torch.zeros(1, dtype=torch.int32, device="cuda")
+        p.cluster(cand, count, gap, events, nev)
+        torch.cuda.synchronize()
+        ev = binding.events_to_numpy(events, nev)
+        snr = rec["env"].astype(np.float64) / rec["sigma"].astype(np.float64)
+        want = oracle.cluster(rec["series"] // w.D, rec["sample"].astype(np.int64), snr, gap)
+        assert int(nev.item()) == len(want) == ev.size
+        for e, o in zip(ev, want):
+            assert (int(e["beam"]), int(e["first_sample"]), int(e["last_sample"]), int(e["count"])) == \
+                   (o["beam"], o["first"], o["last"], o["count"])
+            pk = rec[o["peak"]]
+            if int(e["peak_sample"]) != int(pk["sample"]):        # fp32 vs fp64 ratio: only an exact-tie class may differ
+                assert abs(e["peak_snr"] - snr[o["peak"]]) <= 1e-6 * snr[o["peak"]]
+            else:
+                assert int(e["peak_trial"]) == int(pk["trial"]) and e["peak_env"] == pk["env"]
+                assert abs(e["peak_snr"] - snr[o["peak"]]) <= 1e-6 * snr[o["peak"]]
+        if gap == 0:
+            assert len(want) == n or any(o["count"] > 1 for o in want) is False
+    # hand-built list (the oracle pin's table) through the same call
+    beam = np.array([0, 0, 0, 0, 1, 1, 2, 2, 2])
+    smp = np.array([10, 12, 40, 41, 5, 105, 7, 8, 9])
+    s = np.array([6.5, 7.0, 6.1, 6.1, 9.0, 6.2, 6.3, 8.0, 8.0], dtype=np.float32)
+    raw = np.zeros(9, dtype=binding.CANDIDATE_DTYPE)
+    raw["series"] = beam * w.D
+    raw["sample"] = smp
+    raw["env"] = s
+    raw["sigma"] = 1.0
+    cd = torch.from_numpy(raw.view(np.uint8).reshape(9, 24).copy()).cuda()
+    cn = torch.tensor([9], dtype=torch.int32, device="cuda")
+    events = torch.zeros((16, 48), dtype=torch.uint8, device="cuda")
+    nev = torch.zeros(1, dtype=torch.int32, device="cuda")
+    p.cluster(cd, cn, 10, events, nev)
+    torch.cuda.synchronize()
+    ev = binding.events_to_numpy(events, nev)
+    assert [(int(e["beam"]), int(e["first_sample"]), int(e["last_sample"]), int(e["count"]), int(e["peak_sample"]))
+            for e in ev] == [(0, 10, 12, 2, 12), (0, 40, 41, 2, 40), (1, 5, 5, 1, 5), (1, 105, 105, 1, 105),
+                             (2, 7, 9, 3, 8)]
+    p.destroy()
