@@ -84,6 +84,7 @@ typedef struct {
 } lofar_event;
 
 typedef enum { LOFAR_SIGMA_BLOCK = 0, LOFAR_SIGMA_CAUSAL = 1 } lofar_sigma_mode;
+typedef enum { LOFAR_INV_MATCHED = 0, LOFAR_INV_LSMR = 1 } lofar_inversion;
 
 /* ---- plan ---------------------------------------------------------------------------------
  * BASELINE.json:north_star: "lofar_plan_create(stations, subbands, beams, taps, STEC)".
@@ -117,6 +118,15 @@ LOFAR_API lofar_status lofar_plan_set_input(lofar_plan *plan, lofar_dtype dtype,
  * (e[n] = sqrt(mean of xhat[n-W+1..n]^2), reading A13), candidate buffer capacity. */
 LOFAR_API lofar_status lofar_plan_set_trigger(lofar_plan *plan, double kappa, int env_window,
                                               uint32_t max_candidates);
+/* How the polyphase filter is inverted after the inverse DFT.  LOFAR_INV_MATCHED (default):
+ * one application of the matched synthesis FIR g = 1024 h (= H^T, reading A8; BASELINE.json:north_star).
+ * LOFAR_INV_LSMR: the paper's method -- the FIR system H x = y, which decouples into
+ * one banded system per residue r (rows: the 15 carried slices and the T slices of the block, unknowns:
+ * slices -15 .. T+14, output: slices 0 .. T-1, reading A23), solved by `iterations` (> 0; the paper: ~25)
+ * LSMR iterations from x = 0 with no stopping test.  Costs 4 work vectors of (T+30)*4096 bytes per series
+ * plus the inverse-DFT rows; needs a series buffer (not trigger-only).  The carried state is the same
+ * 15-slice history. */
+LOFAR_API lofar_status lofar_plan_set_inversion(lofar_plan *plan, lofar_inversion mode, int iterations);
 /* Reference level of the trigger (the recovered signal is used "only
  * to trigger the read-out", so the threshold must be known while a block is reconstructed).
  * LOFAR_SIGMA_BLOCK (default): candidates of a block are measured against the envelope RMS of that

@@ -18,6 +18,7 @@ LOFAR_OK, LOFAR_E_INVALID, LOFAR_E_SHAPE, LOFAR_E_ALIGN, LOFAR_E_ALLOC, LOFAR_E_
     LOFAR_E_OVERFLOW, LOFAR_E_STATE = range(8)
 LOFAR_CI8, LOFAR_CI16 = 0, 1
 LOFAR_SIGMA_BLOCK, LOFAR_SIGMA_CAUSAL = 0, 1
+LOFAR_INV_MATCHED, LOFAR_INV_LSMR = 0, 1
 
 # numpy view of lofar_candidate (24 bytes)
 CANDIDATE_DTYPE = np.dtype([("series", "<u4"), ("trial", "<u4"), ("sample", "<u8"),
@@ -32,7 +33,7 @@ assert EVENT_DTYPE.itemsize == 48
 EXPORTS = (
     "lofar_plan_create", "lofar_plan_destroy", "lofar_plan_set_band", "lofar_plan_set_delays",
     "lofar_plan_set_trials", "lofar_plan_set_filter", "lofar_plan_set_input",
-    "lofar_plan_set_trigger", "lofar_plan_set_sigma_mode", "lofar_cluster",
+    "lofar_plan_set_trigger", "lofar_plan_set_sigma_mode", "lofar_plan_set_inversion", "lofar_cluster",
     "lofar_plan_workspace_bytes", "lofar_plan_set_allocator",
     "lofar_plan_set_scratch_limit", "lofar_plan_chunking", "lofar_stream_state_bytes",
     "lofar_stream_get_state", "lofar_stream_set_state", "lofar_beamform_dedisperse",
@@ -72,6 +73,7 @@ def load() -> ctypes.CDLL:
         "lofar_plan_set_input": (i, [vp, i, i]),
         "lofar_plan_set_trigger": (i, [vp, d, i, u32]),
         "lofar_plan_set_sigma_mode": (i, [vp, i, vp]),
+        "lofar_plan_set_inversion": (i, [vp, i, i]),
         "lofar_cluster": (i, [vp, vp, vp, u64, vp, vp, u32, vp]),
         "lofar_plan_workspace_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
         "lofar_plan_set_allocator": (i, [vp, vp, vp, vp]),
@@ -185,6 +187,9 @@ class Plan:
     def set_trigger(self, kappa: float, env_window: int = 1, max_candidates: int = 65536):
         _check(self._lib.lofar_plan_set_trigger(self._h, float(kappa), env_window, max_candidates), "lofar_plan_set_trigger")
         self.max_candidates = max_candidates
+
+    def set_inversion(self, mode: int, iterations: int = 25):
+        _check(self._lib.lofar_plan_set_inversion(self._h, mode, iterations), "lofar_plan_set_inversion")
 
     def set_sigma_mode(self, mode: int, sigma_init=None):
         if sigma_init is None:

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblofar_moon.so")
-SOURCES = ["api.cu", "beamform.cu", "beamform_tc.cu", "ippf.cu", "trigger.cu"]
+SOURCES = ["api.cu", "beamform.cu", "beamform_tc.cu", "ippf.cu", "trigger.cu", "lsmr.cu"]
 HEADERS = ["plan.h", "fft_math.cuh", os.path.join(ROOT, "include", "lofar_moon.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [

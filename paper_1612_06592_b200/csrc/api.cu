@@ -75,6 +75,8 @@ void free_tables(lofar_plan *p)
     dev_free(p, p->dW); dev_free(p, p->dDph); dev_free(p, p->dGs); dev_free(p, p->dTw);
     dev_free(p, p->dHist[0]); dev_free(p, p->dHist[1]); dev_free(p, p->dTail);
     dev_free(p, p->dZ); dev_free(p, p->dPartial); dev_free(p, p->dChunkMax);
+    dev_free(p, p->dY); dev_free(p, p->dLsmrWork); dev_free(p, p->dLsmrPartial);
+    { char *sc = static_cast<char *>(p->dLsmrScal); dev_free(p, sc); p->dLsmrScal = nullptr; }
     dev_free(p, p->dItems); dev_free(p, p->dNItems); dev_free(p, p->dSigmaRef); dev_free(p, p->dThr); dev_free(p, p->dHist0);
     p->have_ref = false;
     free_staging(p);
@@ -137,13 +139,16 @@ size_t sample_bytes(const lofar_plan *p) { return p->dtype == LOFAR_CI16 ? 4 : 2
 struct Layout {
     bool tc;                 // tensor-core operand images wanted (int8 input)
     size_t W, Dph, gs, tw, wimg, hist, tail, Z, partial, chunkmax, items;
+    size_t y, lsmr_work, lsmr_scal_bytes, lsmr_partial;   // LSMR inversion only
+    long long ypitch, wpitch;
     size_t x_bytes, cand, sigma;   // streaming staging (per slot)
     long long cap, zchunk, nsteps;
     size_t table_bytes() const
     {
         return (W + Dph + gs + tw + Z) * sizeof(float2) + wimg * sizeof(unsigned short) +
                (3 * hist + tail + chunkmax + 2 * sigma) * sizeof(float) + partial * sizeof(double) +
-               items * sizeof(int2) + sizeof(uint32_t);
+               items * sizeof(int2) + sizeof(uint32_t) +
+               (y + lsmr_work) * sizeof(float) + lsmr_scal_bytes + lsmr_partial * sizeof(double);
     }
     size_t staging_bytes() const
     {
@@ -170,6 +175,15 @@ Layout layout(const lofar_plan *p)
     L.partial = ns * (size_t)L.nsteps;
     L.chunkmax = ns * (size_t)L.nsteps;
     L.items = 16384;                   // flagged chunks per block before the scan falls back to all of them
+    if (p->inversion == LOFAR_INV_LSMR) {
+        const long long T = p->max_slices > 0 ? p->max_slices : kStepSlices;
+        L.ypitch = (T + kTaps - 1) * kMfft;
+        L.wpitch = (T + 2 * (kTaps - 1)) * kMfft;
+        L.y = ns * (size_t)L.ypitch;
+        L.lsmr_work = 4 * ns * (size_t)L.wpitch;
+        L.lsmr_scal_bytes = lsmr_scalar_bytes((int)ns);
+        L.lsmr_partial = lsmr_partial_count((int)ns, T + 2 * (kTaps - 1));
+    }
     L.x_bytes = S * 2 * K * (size_t)(p->max_slices > 0 ? p->max_slices : 0) * sample_bytes(p);
     L.cand = p->max_cand; L.sigma = ns;
     return L;
@@ -272,6 +286,15 @@ lofar_status build(lofar_plan *p)
     if ((st = dev_alloc(p, &p->dThr, L.sigma)) != LOFAR_OK) return st;
     if ((st = dev_alloc(p, &p->dHist0, L.hist)) != LOFAR_OK) return st;
     CU(cudaMemset(p->dNItems, 0, sizeof(uint32_t)));
+    if (p->inversion == LOFAR_INV_LSMR) {
+        p->ypitch = L.ypitch; p->wpitch = L.wpitch;
+        if ((st = dev_alloc(p, &p->dY, L.y)) != LOFAR_OK) return st;
+        if ((st = dev_alloc(p, &p->dLsmrWork, L.lsmr_work)) != LOFAR_OK) return st;
+        char *sc = nullptr;
+        if ((st = dev_alloc(p, &sc, L.lsmr_scal_bytes)) != LOFAR_OK) return st;
+        p->dLsmrScal = sc;
+        if ((st = dev_alloc(p, &p->dLsmrPartial, L.lsmr_partial)) != LOFAR_OK) return st;
+    }
     if ((st = load_sigma_init(p, nullptr)) != LOFAR_OK) return st;
     CU(cudaDeviceSynchronize());       // build is the one place that may block: tables are in place when it returns
     p->built = true;
@@ -326,14 +349,33 @@ int beamform_dispatch(lofar_plan *p, const BeamformArgs &b, cudaStream_t st)
     return launch_beamform(b, st);
 }
 
+// LSMR inversion (f1): the carried 15 slices of y go in front of the rows the inverse DFT is about to write.
+lofar_status lsmr_begin(lofar_plan *p, cudaStream_t st)
+{
+    const size_t row = (size_t)(kTaps - 1) * kMfft * sizeof(float);
+    CU(cudaMemcpy2DAsync(p->dY, (size_t)p->ypitch * sizeof(float), p->dHist[p->hist_parity], row, row,
+                         (size_t)p->B * p->D, cudaMemcpyDeviceToDevice, st));
+    return LOFAR_OK;
+}
+
+lofar_status lsmr_solve(lofar_plan *p, long long T, float *series, long long series_pitch, cudaStream_t st)
+{
+    const int n = launch_lsmr(p->dY, p->ypitch, T, p->dLsmrWork, p->wpitch, reinterpret_cast<const float *>(p->dGs),
+                              p->dLsmrScal, p->dLsmrPartial, p->B * p->D, p->lsmr_iters, series, series_pitch, st);
+    if (n < 0) return LOFAR_E_CUDA;
+    p->launches += n;
+    return LOFAR_OK;
+}
+
 struct EmitTo { lofar_candidate *cand; uint32_t *count; };   // cand == nullptr: no emission from the epilogue
 
 lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, int ztile, long long nc, int zmap_trials,
                      float *series, long long series_pitch, long long out0, int *partial0, long long step0,
-                     cudaStream_t st, EmitTo em = EmitTo{nullptr, nullptr})
+                     cudaStream_t st, EmitTo em = EmitTo{nullptr, nullptr}, bool y_only = false)
 {
     IppfArgs a{};
     a.D = p->D; a.offset = p->offset;
+    if (y_only) { a.yout = p->dY + (kTaps - 1) * kMfft; a.yout_pitch = p->ypitch; }
     if (em.cand) {
         a.thr = p->dThr; a.sigma_ref = p->dSigmaRef;
         a.cand = em.cand; a.count = em.count; a.cap = p->max_cand;
@@ -394,9 +436,12 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
     //   emit   -- threshold known before the block: decided in the inverse-PPF epilogue;
     //   scan   -- two-pass: sigma of this block, then the stored series is re-read where its maximum allows;
     //   rescan -- two-pass without a series: those places are recomputed from X.
-    const bool emit = causal && p->have_ref;
+    const bool lsmr = p->inversion == LOFAR_INV_LSMR;
+    const bool emit = causal && p->have_ref && !lsmr;      // the LSMR series is thresholded after the solve
     const bool rescan = !emit && series == nullptr;
     if ((causal || series == nullptr) && p->env_window != 1) return LOFAR_E_INVALID;
+    if (lsmr && series == nullptr) return LOFAR_E_INVALID;
+    if (lsmr) { const lofar_status s0 = lsmr_begin(p, st); if (s0 != LOFAR_OK) return s0; }
     if (emit || rescan) CU(cudaMemsetAsync(count, 0, sizeof(uint32_t), st));
     if (rescan)
         CU(cudaMemcpyAsync(p->dHist0, p->dHist[p->hist_parity], (size_t)ns * (kTaps - 1) * kMfft * sizeof(float),
@@ -415,18 +460,20 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
             if (n < 0) return LOFAR_E_CUDA;
             p->launches += n;
         }
-        lofar_status s = do_ippf(p, p->dZ, p->zchunk, 1, nc, p->D > 1 ? p->D : 0, series, N, c0 * kMfft, &partial0,
-                                 c0 / kStepSlices, st, emit ? EmitTo{cand, count} : EmitTo{nullptr, nullptr});
+        lofar_status s = do_ippf(p, p->dZ, p->zchunk, 1, nc, p->D > 1 ? p->D : 0, lsmr ? nullptr : series, N, c0 * kMfft,
+                                 &partial0, c0 / kStepSlices, st, emit ? EmitTo{cand, count} : EmitTo{nullptr, nullptr},
+                                 lsmr);
         if (s != LOFAR_OK) return s;
     }
+    if (lsmr) { const lofar_status s1 = lsmr_solve(p, T, series, N, st); if (s1 != LOFAR_OK) return s1; }
     TriggerArgs t = trigger_args(p, series, N, cand, count, sigma);
     t.zero_count = (emit || rescan) ? 0 : 1;
     int n;
     ProfScope prof(p, 2, st);
-    if (p->env_window == 1) {
+    if (p->env_window == 1 && !lsmr) {
         t.nparts = partial0;
     } else {
-        t.nparts = (int)t.nchunks;
+        t.nparts = (int)t.nchunks;     // sum of squares and chunk maxima recomputed from the series
         if ((n = launch_trigger_reduce(t, st)) < 0) return LOFAR_E_CUDA;
         p->launches += n;
     }
@@ -576,6 +623,16 @@ lofar_status lofar_plan_set_allocator(lofar_plan *p, void *(*alloc)(size_t, void
     return LOFAR_OK;
 }
 
+lofar_status lofar_plan_set_inversion(lofar_plan *p, lofar_inversion mode, int iterations)
+{
+    if (!p || (mode != LOFAR_INV_MATCHED && mode != LOFAR_INV_LSMR)) return LOFAR_E_INVALID;
+    if (mode == LOFAR_INV_LSMR && iterations <= 0) return LOFAR_E_INVALID;
+    p->inversion = mode;
+    if (mode == LOFAR_INV_LSMR) p->lsmr_iters = iterations;
+    p->built = false;
+    return LOFAR_OK;
+}
+
 lofar_status lofar_plan_set_sigma_mode(lofar_plan *p, lofar_sigma_mode mode, const float *sigma_init)
 {
     if (!p || (mode != LOFAR_SIGMA_BLOCK && mode != LOFAR_SIGMA_CAUSAL)) return LOFAR_E_INVALID;
@@ -651,6 +708,13 @@ lofar_status lofar_inverse_ppf(lofar_plan *p, const void *Z, int slices, float *
     if (reinterpret_cast<size_t>(Z) & 7 || reinterpret_cast<size_t>(series) & 7) return LOFAR_E_ALIGN;
     if ((s = apply_reset(p, static_cast<cudaStream_t>(stream))) != LOFAR_OK) return s;
     int partial0 = 0;
+    if (p->inversion == LOFAR_INV_LSMR) {
+        cudaStream_t st = static_cast<cudaStream_t>(stream);
+        if ((s = lsmr_begin(p, st)) != LOFAR_OK) return s;
+        if ((s = do_ippf(p, static_cast<const float2 *>(Z), slices, 0, slices, 0, nullptr, (long long)slices * kMfft, 0,
+                         &partial0, 0, st, EmitTo{nullptr, nullptr}, true)) != LOFAR_OK) return s;
+        return lsmr_solve(p, slices, series, (long long)slices * kMfft, st);
+    }
     return do_ippf(p, static_cast<const float2 *>(Z), slices, 0, slices, 0, series, (long long)slices * kMfft, 0,
                    &partial0, 0, static_cast<cudaStream_t>(stream));
 }

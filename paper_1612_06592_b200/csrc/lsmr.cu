@@ -1,0 +1,213 @@
+// lsmr.cu -- row f1 of SURVEY.md 8(f): least-squares inversion of the polyphase filter by LSMR
+// (section 3: "a system of sparse linear equations H x^ = y where H is the matrix of the FIR
+// filters ... solved by an iterative LSMR algorithm [14] ... convergence ... after approximately 25 iterations";
+// Fong & Saunders; reading A23 in DESIGN.md).
+//
+// H is block diagonal over the 1024 residues: residue r of one series is its own banded system
+//     (A v)[m]   = sum_{t<16} taps[t][r] v[m + t],   m = 0 .. n_eq-1   (n_eq = 15 carried + T slices of y)
+//     (A^T u)[n] = sum_{t<16} taps[t][r] u[n - t],   n = 0 .. n_un-1   (n_un = n_eq + 15 unknown slices)
+// with b = y / 1024.  Every (series, residue) runs the LSMR recurrences with its own scalars; nothing couples
+// them, so the vectors are laid out [row][1024] and a thread owns one residue of a run of rows: loads are
+// coalesced over residues and the 16-tap window slides through registers along the rows.
+// Vectors are kept unnormalised (u', v') next to their norms (beta, alpha): a pass never has to wait for a norm
+// it produces itself.  Norms: per-chunk partial sums in double, added in a fixed order.
+#include "plan.h"
+
+namespace lofar {
+namespace {
+
+constexpr int kTapsN = 16, kRes = 1024, kRows = 64;      // rows per CTA
+constexpr int kLsmrThreads = 256;
+
+// Scalars of one (series, residue), double precision (Fong & Saunders, "Algorithm LSMR", lambda = 0).
+struct Scal {
+    double alpha, beta, alphabar, zetabar, rho, rhobar, cbar, sbar;
+    double inv_alpha, inv_beta;          // 1/alpha, 1/beta of the stored (unnormalised) v', u'
+    double ch, cx, cv;                   // hbar = h - ch hbar; x += cx hbar; h = v - cv h
+};
+
+__device__ __forceinline__ double safe_div(double a, double d) { return d != 0.0 ? a / d : 0.0; }
+
+// u'[m] = sum_t taps[t] v'[m+t] / alpha - alpha * u'[m] / beta_old    (first = 0)
+// or first = 1:  u' = b / 1024 (the right-hand side), nothing else.
+__global__ void __launch_bounds__(kLsmrThreads) u_kernel(float *u, long long upitch, long long n_eq, const float *v,
+                                                         long long vpitch, const float *gs, const Scal *sc, double *partial,
+                                                         int nchunks, int first)
+{
+    const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, series = blockIdx.z;
+    float *pu = u + (size_t)series * upitch + r;
+    const long long m0 = (long long)chunk * kRows, m1 = m0 + kRows < n_eq ? m0 + kRows : n_eq;
+    double s = 0.0;
+    if (first) {
+        for (long long m = m0; m < m1; ++m) {
+            const float val = pu[(size_t)m * kRes] * (1.0f / 1024.0f);
+            pu[(size_t)m * kRes] = val;
+            s += (double)val * val;
+        }
+    } else {
+        const Scal z = sc[(size_t)series * kRes + r];
+        const float ia = (float)z.inv_alpha, ab = (float)(z.alpha * z.inv_beta);
+        const float *pv = v + (size_t)series * vpitch + r;
+        float tap[kTapsN], win[kTapsN];
+#pragma unroll
+        for (int t = 0; t < kTapsN; ++t) tap[t] = gs[t * kRes + r] * (1.0f / 1024.0f);
+#pragma unroll
+        for (int t = 0; t < kTapsN - 1; ++t) win[t + 1] = pv[(size_t)(m0 + t) * kRes];
+        for (long long m = m0; m < m1; ++m) {
+#pragma unroll
+            for (int t = 0; t < kTapsN - 1; ++t) win[t] = win[t + 1];
+            win[kTapsN - 1] = pv[(size_t)(m + kTapsN - 1) * kRes];        // rows m .. m+15 of v' (n_un = n_eq + 15)
+            float acc = 0.f;
+#pragma unroll
+            for (int t = 0; t < kTapsN; ++t) acc = fmaf(tap[t], win[t], acc);
+            const float val = fmaf(acc, ia, -ab * pu[(size_t)m * kRes]);
+            pu[(size_t)m * kRes] = val;
+            s += (double)val * val;
+        }
+    }
+    partial[((size_t)series * nchunks + chunk) * kRes + r] = s;
+}
+
+// v'[n] = sum_t taps[t] u'[n-t] / beta - beta * v'[n] / alpha_old     (first: no second term)
+__global__ void __launch_bounds__(kLsmrThreads) v_kernel(float *v, long long vpitch, long long n_un, const float *u,
+                                                         long long upitch, long long n_eq, const float *gs, const Scal *sc,
+                                                         double *partial, int nchunks, int first)
+{
+    const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, series = blockIdx.z;
+    float *pv = v + (size_t)series * vpitch + r;
+    const float *pu = u + (size_t)series * upitch + r;
+    const long long n0 = (long long)chunk * kRows, n1 = n0 + kRows < n_un ? n0 + kRows : n_un;
+    const Scal z = sc[(size_t)series * kRes + r];
+    const float ib = (float)z.inv_beta, ba = first ? 0.f : (float)(z.beta * z.inv_alpha);
+    float tap[kTapsN], win[kTapsN];       // win[t] = u'[n - t]
+#pragma unroll
+    for (int t = 0; t < kTapsN; ++t) tap[t] = gs[t * kRes + r] * (1.0f / 1024.0f);
+#pragma unroll
+    for (int t = 0; t < kTapsN - 1; ++t) {
+        const long long m = n0 - 1 - t;
+        win[t] = (m >= 0 && m < n_eq) ? pu[(size_t)m * kRes] : 0.f;
+    }
+    double s = 0.0;
+    for (long long n = n0; n < n1; ++n) {
+#pragma unroll
+        for (int t = kTapsN - 1; t > 0; --t) win[t] = win[t - 1];
+        win[0] = n < n_eq ? pu[(size_t)n * kRes] : 0.f;
+        float acc = 0.f;
+#pragma unroll
+        for (int t = 0; t < kTapsN; ++t) acc = fmaf(tap[t], win[t], acc);
+        float val = acc * ib;
+        if (!first) val = fmaf(-ba, pv[(size_t)n * kRes], val);
+        pv[(size_t)n * kRes] = val;
+        s += (double)val * val;
+    }
+    partial[((size_t)series * nchunks + chunk) * kRes + r] = s;
+}
+
+// which: 0 beta_1 (start), 1 alpha_1 + initial scalars, 2 beta_{k+1}, 3 alpha_{k+1} + the plane rotations.
+__global__ void __launch_bounds__(kLsmrThreads) scalar_kernel(Scal *sc, const double *partial, int nchunks, int which)
+{
+    const int r = blockIdx.x * kLsmrThreads + threadIdx.x, series = blockIdx.y;
+    const double *p = partial + (size_t)series * nchunks * kRes + r;
+    double s = 0.0;
+    for (int c = 0; c < nchunks; ++c) s += p[(size_t)c * kRes];
+    const double nrm = sqrt(s);
+    Scal z = sc[(size_t)series * kRes + r];
+    if (which == 0) {
+        z.beta = nrm; z.inv_beta = safe_div(1.0, nrm);
+    } else if (which == 1) {
+        z.alpha = nrm; z.inv_alpha = safe_div(1.0, nrm);
+        z.alphabar = z.alpha; z.zetabar = z.alpha * z.beta;
+        z.rho = 1.0; z.rhobar = 1.0; z.cbar = 1.0; z.sbar = 0.0;
+        z.ch = 0.0; z.cx = 0.0; z.cv = 0.0;
+    } else if (which == 2) {
+        z.beta = nrm; z.inv_beta = safe_div(1.0, nrm);
+    } else {
+        z.alpha = nrm; z.inv_alpha = safe_div(1.0, nrm);
+        const double rhoold = z.rho;
+        z.rho = hypot(z.alphabar, z.beta);
+        const double c = safe_div(z.alphabar, z.rho), s1 = safe_div(z.beta, z.rho);
+        const double thetanew = s1 * z.alpha;
+        z.alphabar = c * z.alpha;
+        const double rhobarold = z.rhobar;
+        const double thetabar = z.sbar * z.rho;
+        const double rhotemp = z.cbar * z.rho;
+        z.rhobar = hypot(rhotemp, thetanew);
+        z.cbar = safe_div(rhotemp, z.rhobar);
+        z.sbar = safe_div(thetanew, z.rhobar);
+        const double zeta = z.cbar * z.zetabar;
+        z.zetabar = -z.sbar * z.zetabar;
+        z.ch = safe_div(thetabar * z.rho, rhoold * rhobarold);
+        z.cx = safe_div(zeta, z.rho * z.rhobar);
+        z.cv = safe_div(thetanew, z.rho);
+    }
+    sc[(size_t)series * kRes + r] = z;
+}
+
+// first: h = v'/alpha, hbar = 0, x = 0.   else: hbar = h - ch hbar; x += cx hbar; h = v'/alpha - cv h.
+__global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, float *x, const float *v, long long pitch,
+                                                         long long n_un, const Scal *sc, int first)
+{
+    const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, series = blockIdx.z;
+    const Scal z = sc[(size_t)series * kRes + r];
+    const float ia = (float)z.inv_alpha, ch = (float)z.ch, cx = (float)z.cx, cv = (float)z.cv;
+    const size_t base = (size_t)series * pitch + r;
+    const long long n0 = (long long)chunk * kRows, n1 = n0 + kRows < n_un ? n0 + kRows : n_un;
+    for (long long n = n0; n < n1; ++n) {
+        const size_t i = base + (size_t)n * kRes;
+        const float vn = v[i] * ia;
+        if (first) { h[i] = vn; hbar[i] = 0.f; x[i] = 0.f; }
+        else {
+            const float hb = fmaf(-ch, hbar[i], h[i]);
+            hbar[i] = hb;
+            x[i] = fmaf(cx, hb, x[i]);
+            h[i] = fmaf(-cv, h[i], vn);
+        }
+    }
+}
+
+// series[q][r] = x[q + 15][r]
+__global__ void __launch_bounds__(kLsmrThreads) out_kernel(const float *x, long long pitch, float *series, long long series_pitch,
+                                                           long long T)
+{
+    const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, s = blockIdx.z;
+    const long long q0 = (long long)chunk * kRows, q1 = q0 + kRows < T ? q0 + kRows : T;
+    for (long long q = q0; q < q1; ++q)
+        series[(size_t)s * series_pitch + (size_t)q * kRes + r] = x[(size_t)s * pitch + (size_t)(q + kTapsN - 1) * kRes + r];
+}
+
+}  // namespace
+
+size_t lsmr_scalar_bytes(int nseries) { return (size_t)nseries * kRes * sizeof(Scal); }
+size_t lsmr_partial_count(int nseries, long long n_un) { return (size_t)nseries * ((n_un + kRows - 1) / kRows) * kRes; }
+
+// y: [nseries][ypitch] floats holding n_eq = 15 + T rows of 1024 (carried history first); overwritten (it becomes u').
+// work: 4 vectors [nseries][wpitch] (v', h, hbar, x), wpitch >= (n_eq + 15) * 1024.  Returns the number of launches.
+int launch_lsmr(float *y, long long ypitch, long long T, float *work, long long wpitch, const float *gs, void *scal,
+                double *partial, int nseries, int iters, float *series, long long series_pitch, cudaStream_t st)
+{
+    const long long n_eq = T + kTapsN - 1, n_un = n_eq + kTapsN - 1;
+    const int ce = (int)((n_eq + kRows - 1) / kRows), cu = (int)((n_un + kRows - 1) / kRows);
+    Scal *sc = static_cast<Scal *>(scal);
+    float *v = work, *h = work + (size_t)nseries * wpitch, *hbar = h + (size_t)nseries * wpitch,
+          *x = hbar + (size_t)nseries * wpitch;
+    const dim3 ge(kRes / kLsmrThreads, ce, nseries), gu(kRes / kLsmrThreads, cu, nseries), gs2(kRes / kLsmrThreads, nseries);
+    int n = 0;
+    cudaMemsetAsync(sc, 0, lsmr_scalar_bytes(nseries), st);
+    u_kernel<<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 1); ++n;
+    scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, ce, 0); ++n;
+    v_kernel<<<gu, kLsmrThreads, 0, st>>>(v, wpitch, n_un, y, ypitch, n_eq, gs, sc, partial, cu, 1); ++n;
+    scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, cu, 1); ++n;
+    h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 1); ++n;
+    for (int k = 0; k < iters; ++k) {
+        u_kernel<<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 0); ++n;
+        scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, ce, 2); ++n;
+        v_kernel<<<gu, kLsmrThreads, 0, st>>>(v, wpitch, n_un, y, ypitch, n_eq, gs, sc, partial, cu, 0); ++n;
+        scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, cu, 3); ++n;
+        h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 0); ++n;
+    }
+    const dim3 go(kRes / kLsmrThreads, (unsigned)((T + kRows - 1) / kRows), nseries);
+    out_kernel<<<go, kLsmrThreads, 0, st>>>(x, wpitch, series, series_pitch, T); ++n;
+    return cudaGetLastError() == cudaSuccess ? n : -1;
+}
+
+}  // namespace lofar

@@ -113,6 +113,11 @@ int launch_beamform_tc(const BeamformArgs &a, const void *wimg, cudaStream_t st)
 int tc_configure();                                     // opt in to the large dynamic shared memory (current device)
 int ippf_configure();                                   // opt in to the large dynamic shared memory
 int launch_rescan(const RescanArgs &a, int grid, cudaStream_t st);
+// LSMR inversion (lsmr.cu)
+size_t lsmr_scalar_bytes(int nseries);
+size_t lsmr_partial_count(int nseries, long long n_un);
+int launch_lsmr(float *y, long long ypitch, long long T, float *work, long long wpitch, const float *gs, void *scal,
+                double *partial, int nseries, int iters, float *series, long long series_pitch, cudaStream_t st);
 int launch_trigger_reduce(const TriggerArgs &a, cudaStream_t st);   // sum e^2 + chunk max from the series
 int launch_trigger_sigma(const TriggerArgs &a, cudaStream_t st);    // sigma from the partial sums
 int launch_trigger_flag(const TriggerArgs &a, cudaStream_t st);     // list of chunks whose maximum can reach the threshold
@@ -136,6 +141,8 @@ struct lofar_plan {
     double kappa = 6.0;
     int env_window = 1;
     uint32_t max_cand = 65536;
+    int inversion = LOFAR_INV_MATCHED;         // f1: LOFAR_INV_LSMR solves H x = y by LSMR instead of applying H^T
+    int lsmr_iters = 25;
     int sigma_mode = LOFAR_SIGMA_BLOCK;        // f3: LOFAR_SIGMA_CAUSAL judges block i against sigma of block i-1
     std::vector<float> sigma_init, thr_init;   // optional reference level of the first block of a stream (and kappa times it)
     // device memory: every plan-owned device buffer goes through these (lofar_plan_set_allocator)
@@ -165,6 +172,10 @@ struct lofar_plan {
     float *dSigmaRef = nullptr, *dThr = nullptr;   // causal sigma: level of the previous block and kappa times it
     bool have_ref = false;
     float *dHist0 = nullptr;           // history at the start of the block (series-free two-pass trigger)
+    float *dY = nullptr, *dLsmrWork = nullptr;     // LSMR: inverse-DFT rows [ns][15+T][1024]; v', h, hbar, x [4][ns][T+30][1024]
+    long long ypitch = 0, wpitch = 0;
+    void *dLsmrScal = nullptr;
+    double *dLsmrPartial = nullptr;
     size_t device_bytes = 0;
     uint64_t offset = 0;
     uint64_t launches = 0;

@@ -192,3 +192,62 @@ def test_cluster_parity(torch, oracle):
             for e in ev] == [(0, 10, 12, 2, 12), (0, 40, 41, 2, 40), (1, 5, 5, 1, 5), (1, 105, 105, 1, 105),
                              (2, 7, 9, 3, 8)]
     p.destroy()
+
+
+# ------------------------------------------------------------------------------------------ f1
+LSMR_TOL = dict(rel=2e-5, mx=2e-4)     # fp32 vectors through 25 iterations (f1): twice north_star's
+
+
+def _close(got, ref, what, rel, mx):
+    got = np.asarray(got, dtype=np.float64)
+    nrm = np.linalg.norm(ref)
+    rms = nrm / np.sqrt(ref.size)
+    err = np.abs(got - ref)
+    assert np.all(np.isfinite(got)), what
+    assert np.linalg.norm(err) / nrm <= rel, f"{what}: rel-L2 {np.linalg.norm(err) / nrm:.3e}"
+    assert err.max() <= mx * rms, f"{what}: max-abs {err.max() / rms:.3e} RMS"
+
+
+@pytest.mark.parametrize("kw,iters", [
+    (dict(S=4, B=2, K=16, k0=300, T=72, dtype="ci16", n_pulses=2, blocks=2, kappa=4.0), 25),
+    (dict(S=4, B=3, K=488, k0=24, T=200, dtype="ci8", n_pulses=3, blocks=2, kappa=4.5), 25),
+    (dict(S=3, B=2, K=24, k0=100, T=40, dtype="ci8", stec=(8.0, 12.0), n_pulses=2, blocks=2, kappa=4.0), 7),
+])
+def test_lsmr_inversion_parity(torch, oracle, kw, iters):
+    """LOFAR_INV_LSMR against O11 (= scipy's lsmr, pinned): whole chain, two blocks (the 15 carried slices are rows of
+    the second block's system), several scratch chunks, sigma and candidates from the LSMR series."""
+    w = synth.small(**kw)
+    tau, blocks = _blocks(w)
+    pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa, inversion="lsmr",
+                                 lsmr_iters=iters)
+    p = binding.plan_for(w, tau)
+    p.set_trigger(w.kappa, 1, 1 << 16)
+    p.set_inversion(binding.LOFAR_INV_LSMR, iters)
+    p.set_scratch_limit(w.B * w.K * 8 * 64)
+    offset = 0
+    for i, X in enumerate(blocks):
+        ref, sig_ref, _, _ = pipe.run_block(X)
+        got, rec, n, sigma, _, _ = _run(torch, p, X, w.T)
+        for s in range(w.nseries):
+            _close(got[s], ref[s], f"block {i} series {s}", LSMR_TOL["rel"], LSMR_TOL["mx"])
+        np.testing.assert_allclose(sigma, sig_ref, rtol=2e-5)
+        env, sig = oracle_snr(oracle, ref, 1)
+        check_candidates(rec, n, env, sig, w.B, w.D, w.kappa, offset)
+        offset += w.T * 1024
+    # the stage call alone, on caller-owned beam sums
+    ns, K, k0, T = 2, 31, 481, 37
+    q = binding.Plan(1, K, ns, 16, 0.0)
+    q.set_band(k0)
+    q.set_input(binding.LOFAR_CI8, T)
+    q.set_inversion(binding.LOFAR_INV_LSMR, 12)
+    Z = synth.random_z(5, ns, K, T)
+    out = torch.empty((ns, T * 1024), dtype=torch.float32, device="cuda")
+    q.inverse_ppf(torch.from_numpy(np.ascontiguousarray(Z.view(np.float32).reshape(ns, K, T, 2))).cuda(), T, out)
+    torch.cuda.synchronize()
+    h = oracle.prototype()
+    for s in range(ns):
+        y = oracle.idft(Z[s].astype(np.complex128), k0)
+        refs = oracle.lsmr_inversion(np.concatenate([np.zeros((15, 1024)), y]), h, 12)
+        _close(out[s].cpu().numpy(), refs, f"stage call series {s}", LSMR_TOL["rel"], LSMR_TOL["mx"])
+    p.destroy()
+    q.destroy()
