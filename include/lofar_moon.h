@@ -85,6 +85,7 @@ typedef struct {
 
 typedef enum { LOFAR_SIGMA_BLOCK = 0, LOFAR_SIGMA_CAUSAL = 1 } lofar_sigma_mode;
 typedef enum { LOFAR_INV_MATCHED = 0, LOFAR_INV_LSMR = 1 } lofar_inversion;
+typedef enum { LOFAR_DEDISP_SUBBAND = 0, LOFAR_DEDISP_EXACT = 1 } lofar_dedispersion;
 
 /* ---- plan ---------------------------------------------------------------------------------
  * BASELINE.json:north_star: "lofar_plan_create(stations, subbands, beams, taps, STEC)".
@@ -127,6 +128,18 @@ LOFAR_API lofar_status lofar_plan_set_trigger(lofar_plan *plan, double kappa, in
  * plus the inverse-DFT rows; needs a series buffer (not trigger-only).  The carried state is the same
  * 15-slice history. */
 LOFAR_API lofar_status lofar_plan_set_inversion(lofar_plan *plan, lofar_inversion mode, int iterations);
+/* Where the ionospheric dispersion is removed.  LOFAR_DEDISP_SUBBAND (default): one phase per
+ * sub-band folded into the beam weight / applied to the beam sums (BASELINE.json:north_star, reading A9).
+ * LOFAR_DEDISP_EXACT: the paper's order -- beams are formed and the polyphase filter is
+ * inverted WITHOUT dispersion phase (one inversion per beam), then every trial multiplies the spectrum of the
+ * 5 ns series by exp(-2 pi i 1.343e9 STEC / f) at the exact frequency of each bin: overlap-save with
+ * 16384-sample transforms of which one slice at either end is discarded (reading A24; valid while the
+ * dispersive delay across the band stays below one slice, STEC <= 40 TECU for the HBA band).  The output
+ * series, sigma and candidate sample indices run ONE SLICE (1024 samples) behind the input: sample n of the
+ * output is time n - 1024 of the stream.  Carried state grows by two slices of the undispersed series per
+ * beam.  Not available in trigger-only mode; lofar_run_block / lofar_stream_push only (the stage calls keep
+ * their definitions). */
+LOFAR_API lofar_status lofar_plan_set_dedispersion(lofar_plan *plan, lofar_dedispersion mode);
 /* Reference level of the trigger (the recovered signal is used "only
  * to trigger the read-out", so the threshold must be known while a block is reconstructed).
  * LOFAR_SIGMA_BLOCK (default): candidates of a block are measured against the envelope RMS of that

@@ -19,6 +19,7 @@ LOFAR_OK, LOFAR_E_INVALID, LOFAR_E_SHAPE, LOFAR_E_ALIGN, LOFAR_E_ALLOC, LOFAR_E_
 LOFAR_CI8, LOFAR_CI16 = 0, 1
 LOFAR_SIGMA_BLOCK, LOFAR_SIGMA_CAUSAL = 0, 1
 LOFAR_INV_MATCHED, LOFAR_INV_LSMR = 0, 1
+LOFAR_DEDISP_SUBBAND, LOFAR_DEDISP_EXACT = 0, 1
 
 # numpy view of lofar_candidate (24 bytes)
 CANDIDATE_DTYPE = np.dtype([("series", "<u4"), ("trial", "<u4"), ("sample", "<u8"),
@@ -33,7 +34,8 @@ assert EVENT_DTYPE.itemsize == 48
 EXPORTS = (
     "lofar_plan_create", "lofar_plan_destroy", "lofar_plan_set_band", "lofar_plan_set_delays",
     "lofar_plan_set_trials", "lofar_plan_set_filter", "lofar_plan_set_input",
-    "lofar_plan_set_trigger", "lofar_plan_set_sigma_mode", "lofar_plan_set_inversion", "lofar_cluster",
+    "lofar_plan_set_trigger", "lofar_plan_set_sigma_mode", "lofar_plan_set_inversion", "lofar_plan_set_dedispersion",
+    "lofar_cluster",
     "lofar_plan_workspace_bytes", "lofar_plan_set_allocator",
     "lofar_plan_set_scratch_limit", "lofar_plan_chunking", "lofar_stream_state_bytes",
     "lofar_stream_get_state", "lofar_stream_set_state", "lofar_beamform_dedisperse",
@@ -74,6 +76,7 @@ def load() -> ctypes.CDLL:
         "lofar_plan_set_trigger": (i, [vp, d, i, u32]),
         "lofar_plan_set_sigma_mode": (i, [vp, i, vp]),
         "lofar_plan_set_inversion": (i, [vp, i, i]),
+        "lofar_plan_set_dedispersion": (i, [vp, i]),
         "lofar_cluster": (i, [vp, vp, vp, u64, vp, vp, u32, vp]),
         "lofar_plan_workspace_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
         "lofar_plan_set_allocator": (i, [vp, vp, vp, vp]),
@@ -190,6 +193,9 @@ class Plan:
 
     def set_inversion(self, mode: int, iterations: int = 25):
         _check(self._lib.lofar_plan_set_inversion(self._h, mode, iterations), "lofar_plan_set_inversion")
+
+    def set_dedispersion(self, mode: int):
+        _check(self._lib.lofar_plan_set_dedispersion(self._h, mode), "lofar_plan_set_dedispersion")
 
     def set_sigma_mode(self, mode: int, sigma_init=None):
         if sigma_init is None:

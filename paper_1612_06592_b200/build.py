@@ -13,8 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblofar_moon.so")
-SOURCES = ["api.cu", "beamform.cu", "beamform_tc.cu", "ippf.cu", "trigger.cu", "lsmr.cu"]
-HEADERS = ["plan.h", "fft_math.cuh", os.path.join(ROOT, "include", "lofar_moon.h")]
+SOURCES = ["api.cu", "beamform.cu", "beamform_tc.cu", "ippf.cu", "trigger.cu", "lsmr.cu", "dedisp.cu"]
+HEADERS = ["plan.h", "fft_math.cuh", "fft_warp.cuh", os.path.join(ROOT, "include", "lofar_moon.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

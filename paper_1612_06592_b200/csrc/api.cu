@@ -75,6 +75,7 @@ void free_tables(lofar_plan *p)
     dev_free(p, p->dW); dev_free(p, p->dDph); dev_free(p, p->dGs); dev_free(p, p->dTw);
     dev_free(p, p->dHist[0]); dev_free(p, p->dHist[1]); dev_free(p, p->dTail);
     dev_free(p, p->dZ); dev_free(p, p->dPartial); dev_free(p, p->dChunkMax);
+    dev_free(p, p->dXhat); dev_free(p, p->dDtab); dev_free(p, p->dTw8192); dev_free(p, p->dTw16k);
     dev_free(p, p->dY); dev_free(p, p->dLsmrWork); dev_free(p, p->dLsmrPartial);
     { char *sc = static_cast<char *>(p->dLsmrScal); dev_free(p, sc); p->dLsmrScal = nullptr; }
     dev_free(p, p->dItems); dev_free(p, p->dNItems); dev_free(p, p->dSigmaRef); dev_free(p, p->dThr); dev_free(p, p->dHist0);
@@ -141,6 +142,8 @@ struct Layout {
     size_t W, Dph, gs, tw, wimg, hist, tail, Z, partial, chunkmax, items;
     size_t y, lsmr_work, lsmr_scal_bytes, lsmr_partial;   // LSMR inversion only
     long long ypitch, wpitch;
+    size_t xhat, dtab, tw8192, tw16k;  // exact de-dispersion only
+    long long xhat_pitch;
     size_t x_bytes, cand, sigma;   // streaming staging (per slot)
     long long cap, zchunk, nsteps;
     size_t table_bytes() const
@@ -148,7 +151,8 @@ struct Layout {
         return (W + Dph + gs + tw + Z) * sizeof(float2) + wimg * sizeof(unsigned short) +
                (3 * hist + tail + chunkmax + 2 * sigma) * sizeof(float) + partial * sizeof(double) +
                items * sizeof(int2) + sizeof(uint32_t) +
-               (y + lsmr_work) * sizeof(float) + lsmr_scal_bytes + lsmr_partial * sizeof(double);
+               (y + lsmr_work + xhat) * sizeof(float) + lsmr_scal_bytes + lsmr_partial * sizeof(double) +
+               (dtab + tw8192 + tw16k) * sizeof(float2);
     }
     size_t staging_bytes() const
     {
@@ -159,11 +163,11 @@ struct Layout {
 Layout layout(const lofar_plan *p)
 {
     Layout L{};
-    const size_t S = p->S, K = p->K, B = p->B, D = p->D, ns = B * D;
+    const size_t S = p->S, K = p->K, B = p->B, D = p->D, ns = B * D, ni = (size_t)p->ninv();
     L.tc = p->dtype == LOFAR_CI8 && p->S <= 32 && p->B <= 128;
     L.W = K * B * S; L.Dph = D * K; L.gs = (size_t)kTaps * kHalf; L.tw = 256 + 512;
     L.wimg = L.tc ? K * 2 * tc_image_halfs(p->S, p->B) : 0;
-    L.hist = ns * (kTaps - 1) * kMfft;
+    L.hist = ni * (kTaps - 1) * kMfft;
     L.tail = ns * (size_t)(p->env_window - 1);
     L.cap = round_up(p->max_slices > 0 ? p->max_slices : kStepSlices, kStepSlices);
     long long zc = (long long)(p->scratch_limit / (B * K * sizeof(float2)));
@@ -179,10 +183,16 @@ Layout layout(const lofar_plan *p)
         const long long T = p->max_slices > 0 ? p->max_slices : kStepSlices;
         L.ypitch = (T + kTaps - 1) * kMfft;
         L.wpitch = (T + 2 * (kTaps - 1)) * kMfft;
-        L.y = ns * (size_t)L.ypitch;
-        L.lsmr_work = 4 * ns * (size_t)L.wpitch;
-        L.lsmr_scal_bytes = lsmr_scalar_bytes((int)ns);
-        L.lsmr_partial = lsmr_partial_count((int)ns, T + 2 * (kTaps - 1));
+        L.y = ni * (size_t)L.ypitch;
+        L.lsmr_work = 4 * ni * (size_t)L.wpitch;
+        L.lsmr_scal_bytes = lsmr_scalar_bytes((int)ni);
+        L.lsmr_partial = lsmr_partial_count((int)ni, T + 2 * (kTaps - 1));
+    }
+    if (p->dedisp == LOFAR_DEDISP_EXACT) {
+        const long long T = p->max_slices > 0 ? p->max_slices : kStepSlices;
+        L.xhat_pitch = (T + 2) * kMfft;
+        L.xhat = B * (size_t)L.xhat_pitch;
+        L.dtab = D * (size_t)8193; L.tw8192 = 8192; L.tw16k = 4097;
     }
     L.x_bytes = S * 2 * K * (size_t)(p->max_slices > 0 ? p->max_slices : 0) * sample_bytes(p);
     L.cand = p->max_cand; L.sigma = ns;
@@ -224,7 +234,8 @@ lofar_status build(lofar_plan *p)
     for (int j = 0; j < K; ++j) {
         const double f = p->f_zone + (double)(p->k0 + j) * (p->clock / kMfft);
         for (int d = 0; d < D; ++d) Dph[(size_t)d * K + j] = unit_phasor(-(kDispersion * p->stec[d] / f));
-        const double fold = (D == 1) ? -(kDispersion * p->stec[0] / f) : 0.0;   // one trial: fold the phase into W
+        // one trial: fold the phase into W (not in exact mode, where the series is de-dispersed after the inversion)
+        const double fold = (D == 1 && p->dedisp != LOFAR_DEDISP_EXACT) ? -(kDispersion * p->stec[0] / f) : 0.0;
         for (int b = 0; b < B; ++b)
             for (int s = 0; s < S; ++s) {
                 double turns = f * p->tau[(size_t)b * S + s] + (fold - std::floor(fold));
@@ -286,6 +297,29 @@ lofar_status build(lofar_plan *p)
     if ((st = dev_alloc(p, &p->dThr, L.sigma)) != LOFAR_OK) return st;
     if ((st = dev_alloc(p, &p->dHist0, L.hist)) != LOFAR_OK) return st;
     CU(cudaMemset(p->dNItems, 0, sizeof(uint32_t)));
+    if (p->dedisp == LOFAR_DEDISP_EXACT) {
+        if (dedisp_configure() != 0) return LOFAR_E_CUDA;
+        p->xhat_pitch = L.xhat_pitch;
+        if ((st = dev_alloc(p, &p->dXhat, L.xhat)) != LOFAR_OK) return st;
+        CU(cudaMemset(p->dXhat, 0, L.xhat * sizeof(float)));
+        std::vector<float2> dt(L.dtab), t8(L.tw8192), t16(L.tw16k);
+        const int nfft = 16 * kMfft;
+        for (int d = 0; d < D; ++d)
+            for (int j = 0; j <= nfft / 2; ++j) {
+                const double fj = p->f_zone + (double)j * (p->clock / nfft);
+                float2 v = unit_phasor(-(kDispersion * p->stec[d] / fj));
+                if (j == 0 || j == nfft / 2) v.y = 0.f;         // the self-conjugate bins keep the real part
+                dt[(size_t)d * 8193 + j] = v;
+            }
+        for (int m = 0; m < 8192; ++m) t8[m] = unit_phasor((double)m / 8192.0);
+        for (int j = 0; j <= 4096; ++j) t16[j] = unit_phasor((double)j / 16384.0);
+        if ((st = dev_alloc(p, &p->dDtab, L.dtab)) != LOFAR_OK) return st;
+        if ((st = dev_alloc(p, &p->dTw8192, L.tw8192)) != LOFAR_OK) return st;
+        if ((st = dev_alloc(p, &p->dTw16k, L.tw16k)) != LOFAR_OK) return st;
+        CU(cudaMemcpy(p->dDtab, dt.data(), dt.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(p->dTw8192, t8.data(), t8.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(p->dTw16k, t16.data(), t16.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    }
     if (p->inversion == LOFAR_INV_LSMR) {
         p->ypitch = L.ypitch; p->wpitch = L.wpitch;
         if ((st = dev_alloc(p, &p->dY, L.y)) != LOFAR_OK) return st;
@@ -305,9 +339,11 @@ lofar_status build(lofar_plan *p)
 lofar_status apply_reset(lofar_plan *p, cudaStream_t st)
 {
     if (!p->reset_pending) return LOFAR_OK;
-    const size_t hist = (size_t)p->B * p->D * (kTaps - 1) * kMfft * sizeof(float);
+    const size_t hist = (size_t)p->ninv() * (kTaps - 1) * kMfft * sizeof(float);
     CU(cudaMemsetAsync(p->dHist[0], 0, hist, st));
     CU(cudaMemsetAsync(p->dHist[1], 0, hist, st));
+    if (p->dXhat)
+        CU(cudaMemset2DAsync(p->dXhat, (size_t)p->xhat_pitch * sizeof(float), 0, 2 * kMfft * sizeof(float), (size_t)p->B, st));
     if (p->dTail) CU(cudaMemsetAsync(p->dTail, 0, (size_t)p->B * p->D * (p->env_window - 1) * sizeof(float), st));
     p->reset_pending = false;
     return load_sigma_init(p, st);
@@ -354,14 +390,14 @@ lofar_status lsmr_begin(lofar_plan *p, cudaStream_t st)
 {
     const size_t row = (size_t)(kTaps - 1) * kMfft * sizeof(float);
     CU(cudaMemcpy2DAsync(p->dY, (size_t)p->ypitch * sizeof(float), p->dHist[p->hist_parity], row, row,
-                         (size_t)p->B * p->D, cudaMemcpyDeviceToDevice, st));
+                         (size_t)p->ninv(), cudaMemcpyDeviceToDevice, st));
     return LOFAR_OK;
 }
 
 lofar_status lsmr_solve(lofar_plan *p, long long T, float *series, long long series_pitch, cudaStream_t st)
 {
     const int n = launch_lsmr(p->dY, p->ypitch, T, p->dLsmrWork, p->wpitch, reinterpret_cast<const float *>(p->dGs),
-                              p->dLsmrScal, p->dLsmrPartial, p->B * p->D, p->lsmr_iters, series, series_pitch, st);
+                              p->dLsmrScal, p->dLsmrPartial, p->ninv(), p->lsmr_iters, series, series_pitch, st);
     if (n < 0) return LOFAR_E_CUDA;
     p->launches += n;
     return LOFAR_OK;
@@ -383,7 +419,7 @@ lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, int ztile
     a.Z = Z; a.zpitch = zpitch; a.ztile = ztile; a.nc = nc;
     a.series = series; a.series_pitch = series_pitch; a.out0 = out0;
     a.Dph = p->dDph; a.zmap_trials = zmap_trials;
-    a.K = p->K; a.k0 = p->k0; a.nseries = p->B * p->D;
+    a.K = p->K; a.k0 = p->k0; a.nseries = p->ninv();
     plan_spans((nc + kStepSlices - 1) / kStepSlices, a.nseries, p->num_sms, &a.nspans, &a.span_len);
     a.hist_in = p->dHist[p->hist_parity];
     a.hist_out = p->dHist[p->hist_parity ^ 1];
@@ -436,8 +472,13 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
     //   emit   -- threshold known before the block: decided in the inverse-PPF epilogue;
     //   scan   -- two-pass: sigma of this block, then the stored series is re-read where its maximum allows;
     //   rescan -- two-pass without a series: those places are recomputed from X.
-    const bool lsmr = p->inversion == LOFAR_INV_LSMR;
-    const bool emit = causal && p->have_ref && !lsmr;      // the LSMR series is thresholded after the solve
+    const bool lsmr = p->inversion == LOFAR_INV_LSMR, exact = p->dedisp == LOFAR_DEDISP_EXACT;
+    const bool emit = causal && p->have_ref && !lsmr && !exact;   // LSMR / exact series are thresholded afterwards
+    if (exact && series == nullptr) return LOFAR_E_INVALID;
+    // exact de-dispersion: the inversion writes the undispersed series of each beam behind its two carried slices
+    float *inv_series = exact ? p->dXhat + 2 * kMfft : series;
+    const long long inv_pitch = exact ? p->xhat_pitch : N;
+    const int ztrials = (p->D > 1 && !exact) ? p->D : 0;
     const bool rescan = !emit && series == nullptr;
     if ((causal || series == nullptr) && p->env_window != 1) return LOFAR_E_INVALID;
     if (lsmr && series == nullptr) return LOFAR_E_INVALID;
@@ -460,17 +501,31 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
             if (n < 0) return LOFAR_E_CUDA;
             p->launches += n;
         }
-        lofar_status s = do_ippf(p, p->dZ, p->zchunk, 1, nc, p->D > 1 ? p->D : 0, lsmr ? nullptr : series, N, c0 * kMfft,
+        lofar_status s = do_ippf(p, p->dZ, p->zchunk, 1, nc, ztrials, lsmr ? nullptr : inv_series, inv_pitch, c0 * kMfft,
                                  &partial0, c0 / kStepSlices, st, emit ? EmitTo{cand, count} : EmitTo{nullptr, nullptr},
                                  lsmr);
         if (s != LOFAR_OK) return s;
     }
-    if (lsmr) { const lofar_status s1 = lsmr_solve(p, T, series, N, st); if (s1 != LOFAR_OK) return s1; }
+    if (lsmr) { const lofar_status s1 = lsmr_solve(p, T, inv_series, inv_pitch, st); if (s1 != LOFAR_OK) return s1; }
+    if (exact) {
+        DedispArgs d{};
+        d.xlead = p->dXhat; d.xpitch = p->xhat_pitch; d.nlead = T + 2;
+        d.series = series; d.series_pitch = N; d.T = T; d.B = p->B; d.D = p->D;
+        d.Dtab = p->dDtab; d.tw8192 = p->dTw8192; d.tw16k = p->dTw16k; d.tw512 = p->dTw + 256;
+        const int nd = launch_dedisp(d, st);
+        if (nd < 0) return LOFAR_E_CUDA;
+        p->launches += nd;
+        // carry the last two slices of the undispersed series (one slice at a time: they may overlap their target)
+        for (int i = 0; i < 2; ++i)
+            CU(cudaMemcpy2DAsync(p->dXhat + (size_t)i * kMfft, (size_t)p->xhat_pitch * sizeof(float),
+                                 p->dXhat + (size_t)(T + i) * kMfft, (size_t)p->xhat_pitch * sizeof(float),
+                                 kMfft * sizeof(float), (size_t)p->B, cudaMemcpyDeviceToDevice, st));
+    }
     TriggerArgs t = trigger_args(p, series, N, cand, count, sigma);
     t.zero_count = (emit || rescan) ? 0 : 1;
     int n;
     ProfScope prof(p, 2, st);
-    if (p->env_window == 1 && !lsmr) {
+    if (p->env_window == 1 && !lsmr && !exact) {
         t.nparts = partial0;
     } else {
         t.nparts = (int)t.nchunks;     // sum of squares and chunk maxima recomputed from the series
@@ -620,6 +675,14 @@ lofar_status lofar_plan_set_allocator(lofar_plan *p, void *(*alloc)(size_t, void
     if (!p || ((alloc == nullptr) != (free_ == nullptr))) return LOFAR_E_INVALID;
     free_tables(p);                    // with the allocator that made them
     p->alloc_fn = alloc; p->free_fn = free_; p->alloc_ctx = ctx;
+    return LOFAR_OK;
+}
+
+lofar_status lofar_plan_set_dedispersion(lofar_plan *p, lofar_dedispersion mode)
+{
+    if (!p || (mode != LOFAR_DEDISP_SUBBAND && mode != LOFAR_DEDISP_EXACT)) return LOFAR_E_INVALID;
+    p->dedisp = mode;
+    p->built = false;
     return LOFAR_OK;
 }
 
@@ -851,9 +914,11 @@ struct StateHeader { uint32_t magic, nseries, taps, fft, env_window, reserved; u
 constexpr uint32_t kStateMagic = 0x4c4f4631u;   // "LOF1"
 size_t state_bytes(const lofar_plan *p)
 {
-    const size_t ns = (size_t)p->B * p->D;
-    return sizeof(StateHeader) + ns * (kTaps - 1) * kMfft * sizeof(float) + ns * (size_t)(p->env_window - 1) * sizeof(float) +
-           ns * sizeof(float);                 // + the causal reference level (header.reserved = 1 if valid)
+    const size_t ns = (size_t)p->B * p->D, ni = (size_t)p->ninv();
+    const size_t xt = p->dedisp == LOFAR_DEDISP_EXACT ? (size_t)p->B * 2 * kMfft : 0;   // exact de-dispersion: two slices per beam
+    return sizeof(StateHeader) + ni * (kTaps - 1) * kMfft * sizeof(float) + ns * (size_t)(p->env_window - 1) * sizeof(float) +
+           ns * sizeof(float) +                // the causal reference level (header.reserved = 1 if valid)
+           xt * sizeof(float);
 }
 }  // namespace
 
@@ -874,14 +939,17 @@ lofar_status lofar_stream_get_state(lofar_plan *p, void *state_host, size_t byte
         if (st != LOFAR_OK) { free_tables(p); return st; }
     }
     quiesce(p);
-    const size_t ns = (size_t)p->B * p->D, hist = ns * (kTaps - 1) * kMfft * sizeof(float);
+    const size_t ns = (size_t)p->B * p->D, hist = (size_t)p->ninv() * (kTaps - 1) * kMfft * sizeof(float);
     const size_t tail = ns * (size_t)(p->env_window - 1) * sizeof(float);
+    const size_t xt = p->dXhat ? (size_t)2 * kMfft * sizeof(float) : 0;
     StateHeader h{kStateMagic, (uint32_t)ns, (uint32_t)kTaps, (uint32_t)kMfft, (uint32_t)p->env_window,
                   (p->have_ref && !p->reset_pending) ? 1u : 0u, p->offset};
     char *dst = static_cast<char *>(state_host);
     std::memcpy(dst, &h, sizeof(h));
-    std::memset(dst + sizeof(h), 0, hist + tail + ns * sizeof(float));
+    std::memset(dst + sizeof(h), 0, hist + tail + ns * sizeof(float) + xt * p->B);
     if (p->reset_pending) return LOFAR_OK;
+    if (xt) CU(cudaMemcpy2D(dst + sizeof(h) + hist + tail + ns * sizeof(float), xt, p->dXhat,
+                            (size_t)p->xhat_pitch * sizeof(float), xt, (size_t)p->B, cudaMemcpyDeviceToHost));
     CU(cudaMemcpy(dst + sizeof(h), p->dHist[p->hist_parity], hist, cudaMemcpyDeviceToHost));
     if (tail) CU(cudaMemcpy(dst + sizeof(h) + hist, p->dTail, tail, cudaMemcpyDeviceToHost));
     if (h.reserved) CU(cudaMemcpy(dst + sizeof(h) + hist + tail, p->dSigmaRef, ns * sizeof(float), cudaMemcpyDeviceToHost));
@@ -904,8 +972,13 @@ lofar_status lofar_stream_set_state(lofar_plan *p, const void *state_host, size_
         if (st != LOFAR_OK) { free_tables(p); return st; }
     }
     quiesce(p);
-    const size_t hist = ns * (kTaps - 1) * kMfft * sizeof(float), tail = ns * (size_t)(p->env_window - 1) * sizeof(float);
+    const size_t hist = (size_t)p->ninv() * (kTaps - 1) * kMfft * sizeof(float), tail = ns * (size_t)(p->env_window - 1) * sizeof(float);
     const char *src = static_cast<const char *>(state_host);
+    if (p->dXhat) {
+        const size_t xt = (size_t)2 * kMfft * sizeof(float);
+        CU(cudaMemcpy2D(p->dXhat, (size_t)p->xhat_pitch * sizeof(float), src + sizeof(h) + hist + tail + ns * sizeof(float), xt,
+                        xt, (size_t)p->B, cudaMemcpyHostToDevice));
+    }
     CU(cudaMemcpy(p->dHist[p->hist_parity], src + sizeof(h), hist, cudaMemcpyHostToDevice));
     if (tail) CU(cudaMemcpy(p->dTail, src + sizeof(h) + hist, tail, cudaMemcpyHostToDevice));
     p->have_ref = false;

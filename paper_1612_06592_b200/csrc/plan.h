@@ -102,6 +102,19 @@ struct TriggerArgs {
 };
 
 
+// Exact de-dispersion (dedisp.cu, f2)
+struct DedispArgs {
+    const float *xlead;   // [B][xpitch]: two carried slices, then the T slices of this block (undispersed xhat)
+    long long xpitch, nlead;   // nlead = T + 2 slices
+    float *series;        // [B*D][series_pitch]: output, one slice behind the input
+    long long series_pitch, T;
+    int B, D;
+    const float2 *Dtab;   // [D][8193] exp(-2 pi i 1.343e9 STEC_d / f_j)
+    const float2 *tw8192; // [8192] exp(2 pi i m / 8192)
+    const float2 *tw16k;  // [4097] exp(2 pi i j / 16384)
+    const float2 *tw512;  // TB[32][16] of the 512-point FFT
+};
+
 // kernel launchers (each returns the number of kernels it launched, or -1 on a launch error)
 int launch_beamform(const BeamformArgs &a, cudaStream_t st);
 int launch_ippf(const IppfArgs &a, cudaStream_t st);
@@ -113,6 +126,8 @@ int launch_beamform_tc(const BeamformArgs &a, const void *wimg, cudaStream_t st)
 int tc_configure();                                     // opt in to the large dynamic shared memory (current device)
 int ippf_configure();                                   // opt in to the large dynamic shared memory
 int launch_rescan(const RescanArgs &a, int grid, cudaStream_t st);
+int dedisp_configure();
+int launch_dedisp(const DedispArgs &a, cudaStream_t st);
 // LSMR inversion (lsmr.cu)
 size_t lsmr_scalar_bytes(int nseries);
 size_t lsmr_partial_count(int nseries, long long n_un);
@@ -132,6 +147,7 @@ int launch_tail_save(const float *series, long long pitch, long long N, int nser
 }  // namespace lofar
 
 struct lofar_plan {
+    int ninv() const { return dedisp == LOFAR_DEDISP_EXACT ? B : B * D; }   // series through the inverse PPF
     // problem
     int S = 0, K = 0, B = 0, D = 1, P = 16, M = 1024, k0 = 0;
     double f_zone = 100e6, clock = 200e6;
@@ -141,6 +157,7 @@ struct lofar_plan {
     double kappa = 6.0;
     int env_window = 1;
     uint32_t max_cand = 65536;
+    int dedisp = LOFAR_DEDISP_SUBBAND;         // f2: LOFAR_DEDISP_EXACT de-disperses the reconstructed 5 ns series per trial
     int inversion = LOFAR_INV_MATCHED;         // f1: LOFAR_INV_LSMR solves H x = y by LSMR instead of applying H^T
     int lsmr_iters = 25;
     int sigma_mode = LOFAR_SIGMA_BLOCK;        // f3: LOFAR_SIGMA_CAUSAL judges block i against sigma of block i-1
@@ -175,6 +192,9 @@ struct lofar_plan {
     float *dY = nullptr, *dLsmrWork = nullptr;     // LSMR: inverse-DFT rows [ns][15+T][1024]; v', h, hbar, x [4][ns][T+30][1024]
     long long ypitch = 0, wpitch = 0;
     void *dLsmrScal = nullptr;
+    float *dXhat = nullptr;            // exact de-dispersion: [B][2 + T][1024] undispersed series behind two carried slices
+    long long xhat_pitch = 0;
+    float2 *dDtab = nullptr, *dTw8192 = nullptr, *dTw16k = nullptr;
     double *dLsmrPartial = nullptr;
     size_t device_bytes = 0;
     uint64_t offset = 0;

@@ -251,3 +251,54 @@ def test_lsmr_inversion_parity(torch, oracle, kw, iters):
         _close(out[s].cpu().numpy(), refs, f"stage call series {s}", LSMR_TOL["rel"], LSMR_TOL["mx"])
     p.destroy()
     q.destroy()
+
+
+# ------------------------------------------------------------------------------------------ f2
+@pytest.mark.parametrize("kw,lsmr", [
+    (dict(S=4, B=2, K=488, k0=24, T=104, dtype="ci8", stec=(12.0,), pulse_stec=12.0, n_pulses=3, blocks=3, kappa=4.5), False),
+    (dict(S=3, B=2, K=64, k0=200, T=44, dtype="ci16", stec=(8.0, 10.0, 12.0), pulse_stec=10.0, n_pulses=3, blocks=2, kappa=4.0), False),
+    (dict(S=3, B=1, K=100, k0=300, T=32, dtype="ci8", stec=(10.0, 20.0), pulse_stec=10.0, n_pulses=2, blocks=2, kappa=4.0), True),
+])
+def test_exact_dedispersion_parity(torch, oracle, kw, lsmr):
+    """LOFAR_DEDISP_EXACT against O12 (overlap-save rfft * D * irfft per trial on the series reconstructed without
+    dispersion phase), whole chain, consecutive blocks (two carried slices of the undispersed series + the PPF
+    history), T not a multiple of the 14-slice hop; once combined with the LSMR inversion."""
+    w = synth.small(**kw)
+    tau, blocks = _blocks(w)
+    pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa, dedisp="exact",
+                                 inversion="lsmr" if lsmr else "matched", lsmr_iters=9)
+    p = binding.plan_for(w, tau)
+    p.set_trigger(w.kappa, 1, 1 << 16)
+    p.set_dedispersion(binding.LOFAR_DEDISP_EXACT)
+    if lsmr:
+        p.set_inversion(binding.LOFAR_INV_LSMR, 9)
+    p.set_scratch_limit(w.B * w.K * 8 * 32)
+    tol = LSMR_TOL if lsmr else dict(rel=1e-5, mx=1e-4)
+    offset = 0
+    state = None
+    for i, X in enumerate(blocks):
+        ref, sig_ref, _, _ = pipe.run_block(X)
+        got, rec, n, sigma, _, _ = _run(torch, p, X, w.T)
+        for s in range(w.nseries):
+            _close(got[s], ref[s], f"block {i} series {s}", tol["rel"], tol["mx"])
+        np.testing.assert_allclose(sigma, sig_ref, rtol=2e-5)
+        env, sig = oracle_snr(oracle, ref, 1)
+        check_candidates(rec, n, env, sig, w.B, w.D, w.kappa, offset)
+        offset += w.T * 1024
+        if i == 0:
+            state = p.get_state()
+            second = got
+    # resume from the checkpoint taken after block 0: the two carried slices travel with the state
+    q = binding.plan_for(w, tau)
+    q.set_trigger(w.kappa, 1, 1 << 16)
+    q.set_dedispersion(binding.LOFAR_DEDISP_EXACT)
+    if lsmr:
+        q.set_inversion(binding.LOFAR_INV_LSMR, 9)
+    q.set_state(state)
+    got_q, _, _, _, _, _ = _run(torch, q, blocks[1], w.T)
+    p.stream_reset()
+    _run(torch, p, blocks[0], w.T)
+    got_p, _, _, _, _, _ = _run(torch, p, blocks[1], w.T)
+    assert np.array_equal(got_q, got_p)
+    p.destroy()
+    q.destroy()
