@@ -181,6 +181,13 @@ LOFAR_API lofar_status lofar_plan_chunking(lofar_plan *plan, int slices, int64_t
 /* a1 + a2:  Z[b*D+d][k][q] = Dph[d,k] * sum_s sum_p W[b,s,k] X[s,p,k,q]. */
 LOFAR_API lofar_status lofar_beamform_dedisperse(lofar_plan *plan, const void *X, int slices,
                                                  void *Z, void *stream);
+/* f4, two-stage beamforming (sub-arrays pre-beamformed on the first cluster, the
+ * final beams formed from those on the second; 16-bit integers on the wire).  Turns the output Z
+ * [B*D][K][slices] float2 of lofar_beamform_dedisperse into the input of a second plan whose "stations" are
+ * these B*D first-stage beams: X2 [B*D][2][K][slices][re,im] int16, polarisation 0 = clip(rint(Z * scale),
+ * +-32767) with ties to even, polarisation 1 = 0.  Device pointers; X2 16-byte aligned. */
+LOFAR_API lofar_status lofar_requantize(lofar_plan *plan, const void *Z, int slices, float scale, void *X2,
+                                        void *stream);
 /* a3 + a4: per series and slice an unnormalised 1024-point Hermitian inverse
  * DFT of the K selected bins (all other bins zero), then
  * xhat[q*1024+r] = 1024 * sum_{t<16} h[r+1024 t] * y[q-t][r].  Reads and then replaces the

@@ -35,7 +35,7 @@ EXPORTS = (
     "lofar_plan_create", "lofar_plan_destroy", "lofar_plan_set_band", "lofar_plan_set_delays",
     "lofar_plan_set_trials", "lofar_plan_set_filter", "lofar_plan_set_input",
     "lofar_plan_set_trigger", "lofar_plan_set_sigma_mode", "lofar_plan_set_inversion", "lofar_plan_set_dedispersion",
-    "lofar_cluster",
+    "lofar_cluster", "lofar_requantize",
     "lofar_plan_workspace_bytes", "lofar_plan_set_allocator",
     "lofar_plan_set_scratch_limit", "lofar_plan_chunking", "lofar_stream_state_bytes",
     "lofar_stream_get_state", "lofar_stream_set_state", "lofar_beamform_dedisperse",
@@ -78,6 +78,7 @@ def load() -> ctypes.CDLL:
         "lofar_plan_set_inversion": (i, [vp, i, i]),
         "lofar_plan_set_dedispersion": (i, [vp, i]),
         "lofar_cluster": (i, [vp, vp, vp, u64, vp, vp, u32, vp]),
+        "lofar_requantize": (i, [vp, vp, i, c.c_float, vp, vp]),
         "lofar_plan_workspace_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
         "lofar_plan_set_allocator": (i, [vp, vp, vp, vp]),
         "lofar_plan_set_scratch_limit": (i, [vp, c.c_size_t]),
@@ -274,6 +275,10 @@ class Plan:
     def beamform_dedisperse(self, X, slices: int, Z, stream=None, allow=()):
         return _check(self._lib.lofar_beamform_dedisperse(self._h, _ptr(X), slices, _ptr(Z), _stream_ptr(stream)),
                       "lofar_beamform_dedisperse", allow)
+
+    def requantize(self, Z, slices: int, scale: float, X2, stream=None, allow=()):
+        return _check(self._lib.lofar_requantize(self._h, _ptr(Z), slices, float(scale), _ptr(X2), _stream_ptr(stream)),
+                      "lofar_requantize", allow)
 
     def inverse_ppf(self, Z, slices: int, series, stream=None, allow=()):
         return _check(self._lib.lofar_inverse_ppf(self._h, _ptr(Z), slices, _ptr(series), _stream_ptr(stream)),

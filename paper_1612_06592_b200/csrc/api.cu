@@ -763,6 +763,17 @@ lofar_status lofar_beamform_dedisperse(lofar_plan *p, const void *X, int slices,
     return LOFAR_OK;
 }
 
+lofar_status lofar_requantize(lofar_plan *p, const void *Z, int slices, float scale, void *X2, void *stream)
+{
+    if (!p || !Z || !X2 || slices <= 0 || !(scale > 0.f)) return LOFAR_E_INVALID;
+    if ((reinterpret_cast<size_t>(Z) & 7) || (reinterpret_cast<size_t>(X2) & 15)) return LOFAR_E_ALIGN;
+    const int n = launch_requantize(static_cast<const float2 *>(Z), (long long)p->K * slices, p->B * p->D, scale, X2,
+                                    static_cast<cudaStream_t>(stream));
+    if (n < 0) return LOFAR_E_CUDA;
+    p->launches += n;
+    return LOFAR_OK;
+}
+
 lofar_status lofar_inverse_ppf(lofar_plan *p, const void *Z, int slices, float *series, void *stream)
 {
     lofar_status s = ensure(p, slices);

@@ -188,7 +188,29 @@ int launch_bt(const BeamformArgs &a, cudaStream_t st)
     return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }
 
+// Two-stage beamforming: the first-stage beams leave as 16-bit integers.
+// Z[g][k][q] float2 -> X2[g][pol 0][k][q] = clip(rint(Z * scale)) (ties to even), pol 1 = 0.
+__global__ void __launch_bounds__(256) requantize_kernel(const float2 *Z, long long n_per_g, int G, float scale, short2 *X2)
+{
+    const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
+    const int g = blockIdx.y;
+    if (i >= n_per_g) return;
+    const float2 z = Z[(size_t)g * n_per_g + i];
+    const int re = max(-32767, min(32767, __float2int_rn(z.x * scale)));
+    const int im = max(-32767, min(32767, __float2int_rn(z.y * scale)));
+    X2[(size_t)(2 * g) * n_per_g + i] = make_short2((short)re, (short)im);
+    X2[(size_t)(2 * g + 1) * n_per_g + i] = make_short2(0, 0);
+}
+
 }  // namespace
+
+int launch_requantize(const float2 *Z, long long n_per_g, int G, float scale, void *X2, cudaStream_t st)
+{
+    if (n_per_g <= 0) return 0;
+    dim3 grid((unsigned)((n_per_g + 255) / 256), (unsigned)G);
+    requantize_kernel<<<grid, 256, 0, st>>>(Z, n_per_g, G, scale, static_cast<short2 *>(X2));
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}
 
 int launch_beamform(const BeamformArgs &a, cudaStream_t st)
 {

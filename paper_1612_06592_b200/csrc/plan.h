@@ -118,6 +118,7 @@ struct DedispArgs {
 // kernel launchers (each returns the number of kernels it launched, or -1 on a launch error)
 int launch_beamform(const BeamformArgs &a, cudaStream_t st);
 int launch_ippf(const IppfArgs &a, cudaStream_t st);
+int launch_requantize(const float2 *Z, long long n_per_g, int G, float scale, void *X2, cudaStream_t st);
 // tensor-core beamformer (beamform_tc.cu)
 bool tc_supported(const BeamformArgs &a);
 size_t tc_image_halfs(int S, int B);

@@ -302,3 +302,61 @@ def test_exact_dedispersion_parity(torch, oracle, kw, lsmr):
     assert np.array_equal(got_q, got_p)
     p.destroy()
     q.destroy()
+
+
+# ------------------------------------------------------------------------------------------ f4
+def test_two_stage_beamforming_parity(torch, oracle):
+    """stage 1 forms one pre-beam per sub-array (its stations summed towards the pointing centre),
+    lofar_requantize turns those into int16 pseudo-stations, stage 2 runs the whole chain on them.
+    Against the oracle doing the same two stages (O4, O13, O4..O8), element by element."""
+    w = synth.small(S=6, B=3, K=24, k0=150, T=72, dtype="ci8", stec=(10.0,), n_pulses=2, kappa=4.0)
+    tau, blocks = _blocks(w)
+    X = blocks[0]
+    groups = [(0, 1, 2), (3, 4, 5)]
+    scale = 16.0
+    tau2 = np.stack([tau[:, list(st)].mean(axis=1) for st in groups], axis=1)          # [B][G]
+    # ---- oracle: stage 1 per group (unit weights, no dispersion), re-quantise, stage 2 chain
+    X2_ref = np.zeros((len(groups), 2, w.K, w.T, 2), dtype=np.int16)
+    W1, D1 = oracle.tables(np.zeros((1, 3)), np.zeros(1), w.K, w.k0)
+    for g, st in enumerate(groups):
+        Zg = oracle.beamform(np.ascontiguousarray(X[list(st)]), W1, D1)
+        X2_ref[g, 0] = oracle.requantise(Zg[0], scale)
+    pipe = oracle.OraclePipeline(tau=tau2, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa)
+    ref, sig_ref, _, _ = pipe.run_block(X2_ref)
+    # ---- GPU: one stage-1 plan per group, lofar_requantize into the stage-2 input, stage-2 plan on int16
+    X2 = torch.zeros((len(groups), 2, w.K, w.T, 2), dtype=torch.int16, device="cuda")
+    for g, st in enumerate(groups):
+        p1 = binding.Plan(3, w.K, 1, 16, 0.0)
+        p1.set_band(w.k0)
+        p1.set_delays(np.zeros((1, 3)))
+        p1.set_input(binding.LOFAR_CI8, w.T)
+        Z = torch.empty((1, w.K, w.T, 2), dtype=torch.float32, device="cuda")
+        p1.beamform_dedisperse(torch.from_numpy(np.ascontiguousarray(X[list(st)])).cuda(), w.T, Z)
+        p1.requantize(Z, w.T, scale, X2[g])
+        torch.cuda.synchronize()
+        p1.destroy()
+    assert np.array_equal(X2.cpu().numpy(), X2_ref)                 # integers: bit-exact
+    p2 = binding.Plan(len(groups), w.K, w.B, 16, w.stec[0])
+    p2.set_band(w.k0)
+    p2.set_delays(tau2)
+    p2.set_input(binding.LOFAR_CI16, w.T)
+    p2.set_trigger(w.kappa, 1, 1 << 16)
+    series, cand, count, sigma = binding.new_outputs(p2, w.T)
+    p2.run_block(X2, w.T, series, cand, count, sigma)
+    torch.cuda.synchronize()
+    got = series.cpu().numpy()
+    for s in range(w.B):
+        assert_close(got[s], ref[s], f"series {s}")
+    np.testing.assert_allclose(sigma.cpu().numpy(), sig_ref, rtol=5e-6)
+    env, sig = oracle_snr(oracle, ref, 1)
+    check_candidates(binding.candidates_to_numpy(cand, count), int(count.item()), env, sig, w.B, 1, w.kappa)
+    # ties to even and clipping of the re-quantiser on hand-made values
+    z = torch.tensor([[0.5, 1.5], [2.5, -0.5], [1e9, -1e9], [-0.49, 0.51]], dtype=torch.float32, device="cuda")
+    q = binding.Plan(1, 1, 1, 16, 0.0)
+    q.set_input(binding.LOFAR_CI16, 4)
+    out = torch.zeros((1, 2, 1, 4, 2), dtype=torch.int16, device="cuda")
+    q.requantize(z.reshape(1, 1, 4, 2), 4, 1.0, out)
+    torch.cuda.synchronize()
+    assert out[0, 0, 0].cpu().tolist() == [[0, 2], [2, 0], [32767, -32767], [0, 1]] and int(out[0, 1].abs().sum()) == 0
+    p2.destroy()
+    q.destroy()
