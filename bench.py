@@ -2,13 +2,20 @@
 """bench.py -- throughput of the whole hot path (beamform+de-dispersion -> inverse PPF -> trigger) on
 synthetic LOFAR-shaped data, per the driver contract.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config i] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config i | --all-configs]
+                    [--mode series|trigger_only|causal|lsmr|exact] [--parallel replicas|beams] [--impl reference]
 
 A step is one lofar_run_block over one block of the workload (default: BASELINE.json:configs[2], the
 24 stations x 488 sub-bands x 24 beams case the north_star target names).  `value` is reconstructed
 5 ns samples/s per beam with the input resident in HBM; `e2e` is the same through lofar_stream_push
-with the block in pinned HOST memory (H2D inside the timed region, candidates/sigma copied back).
-N > 1: the path has no sharding or collectives (north_star) -> N independent replicas, one per GPU.
+with the blocks in pinned HOST memory (H2D inside the timed region, candidates/sigma copied back); for
+configs[4] the e2e leg is the configuration BASELINE.json states: 10 consecutive blocks of 195312 slices.
+`--mode` selects the rows "next" of SURVEY.md 8(f): trigger_only (series == NULL), causal (sigma of the
+previous block, series-free), lsmr (LSMR inversion, 25 iterations), exact (paper-order de-dispersion).
+N > 1: `--parallel replicas` (default; north_star: no sharding or collectives -> N independent replicas, weak
+scaling) or `--parallel beams` (f4: the beams are split over the ranks and every step starts with an NCCL
+broadcast of the input block from rank 0; strong scaling).  `--gpus N` without a torchrun environment
+re-launches itself under torch.distributed.run.
 `--impl reference` times the CPU oracle on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -16,6 +23,7 @@ from __future__ import annotations
 import argparse
 import json
 import os
+import platform
 import subprocess
 import sys
 import tempfile
@@ -27,10 +35,11 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_1612_06592_b200 import synth  # noqa: E402
+from paper_1612_06592_b200 import shard, synth  # noqa: E402
 
 METRIC = "reconstructed 5 ns samples/s per beam"
 UNIT = "samples/s/beam"
+MODES = ("series", "trigger_only", "causal", "lsmr", "exact")
 
 
 def peaks():
@@ -39,6 +48,14 @@ def peaks():
         d = json.load(open(path))
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_summary():
+    """dram traffic / limiter per kernel from the committed ncu post-processing (profile_summary.py)."""
+    path = os.path.join(ROOT, "profiles", "ncu_summary.json")
+    if os.path.exists(path):
+        return json.load(open(path))
+    return {}
 
 
 def workload(idx: int, slices: int | None):
@@ -54,7 +71,7 @@ def describe(w, extra=None):
                      f"T={w.T} slices/block {w.dtype}",
          "stations": w.S, "beams": w.B, "trials": w.D, "subbands": w.K, "slices_per_block": w.T,
          "input_dtype": w.dtype, "block_seconds_of_data": w.T * w.slice_seconds,
-         "l2": "inputs larger than L2 (no flush needed)" if w.input_bytes > 256e6 else "flushed"}
+         "l2": "inputs larger than L2 (no flush needed)" if w.input_bytes > 256e6 else "L2 flushed between steps"}
     if extra:
         d.update(extra)
     return d
@@ -97,24 +114,60 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return platform.processor() or "unknown"
+
+
 # ------------------------------------------------------------------------------------- oracle legs
-def oracle_sample(w, X_sample, tau, budget_s=15.0):
+def oracle_pipe(oracle, w, tau, mode):
+    kw = {}
+    if mode == "lsmr":
+        kw = dict(inversion="lsmr", lsmr_iters=25)
+    elif mode == "exact":
+        kw = dict(dedisp="exact")
+    elif mode == "causal":
+        kw = dict(sigma_mode="causal")
+    return oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa, **kw)
+
+
+def oracle_sample(w, X_sample, tau, budget_s=15.0, mode="series", threads=None):
     """Times the oracle as it stands on a bounded sample (the first `nq` slices of the block, all
     stations/sub-bands/beams/trials); returns (samples/s/beam, cores, description, seconds)."""
     from oracle import lofar_oracle as oracle
-    pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa)
-    nq = 4
+    if threads:
+        oracle.set_threads(threads)
+    pipe = oracle_pipe(oracle, w, tau, mode)
+    nq = 8
     t0 = time.perf_counter()
     pipe.run_block(np.ascontiguousarray(X_sample[:, :, :, :nq]))
     probe = time.perf_counter() - t0
     per_slice = max(probe / nq, 1e-6)
-    nq = int(min(X_sample.shape[3], max(8, budget_s / per_slice)))
+    nq = int(min(X_sample.shape[3], max(8, budget_s / per_slice))) // 8 * 8
     pipe.reset()
     xs = np.ascontiguousarray(X_sample[:, :, :, :nq])
     t0 = time.perf_counter()
     pipe.run_block(xs)
     dt = time.perf_counter() - t0
     return nq * w.M / dt, oracle.threads(), f"first {nq} slices of one block, all {w.nseries} series", dt
+
+
+def cpu_baseline(w, X, tau, mode, budget_s=10.0):
+    from oracle import lofar_oracle as oracle
+    ncores = os.cpu_count() or 1
+    v, cores, sample, dt = oracle_sample(w, X, tau, budget_s, mode, threads=ncores)
+    v1, _, sample1, dt1 = oracle_sample(w, X, tau, budget_s / 2, mode, threads=1)
+    oracle.set_threads(ncores)
+    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt,
+            "single_thread": {"value": v1, "cores": 1, "sample": sample1, "seconds": dt1},
+            "cpu_model": cpu_model(), "build": oracle.BUILD_FLAGS,
+            "note": "oracle/ as it stands (fp64, naive O(M*K) inverse DFT, direct convolution); a reported baseline, "
+                    "not the target"}
 
 
 def run_reference(args):
@@ -129,18 +182,20 @@ def run_reference(args):
     vals, cores, sample = [], 1, ""
     budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     for i in range(args.warmup + args.steps):
-        v, cores, sample, dt = oracle_sample(w, X, tau, budget)
+        v, cores, sample, dt = oracle_sample(w, X, tau, budget, args.mode)
         if i >= args.warmup:
             vals.append((v, dt))
     value = float(np.mean([v for v, _ in vals]))
     ms = float(np.mean([dt for _, dt in vals]) * 1e3)
+    from oracle import lofar_oracle as oracle
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, paper_1612_06592_b200.synth)",
-        "config": describe(w, {"note": "each step is a bounded sample of the block"}),
+        "config": describe(w, {"mode": args.mode, "note": "each step is a bounded sample of the block"}),
         "real_time_factor": value / 200e6,
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "cpu_model": cpu_model(), "build": oracle.BUILD_FLAGS},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
@@ -148,9 +203,7 @@ def run_reference(args):
 
 # ------------------------------------------------------------------------------------- replicas
 def max_over_ranks(value: float, dist, device="cpu") -> float:
-    """MAX over ranks of a per-rank duration (the contract's multi-GPU timing rule).  The path has no
-    sharding or collectives (north_star: "replicas only"), so this and the barrier are the only
-    cross-rank operations in the bench."""
+    """MAX over ranks of a per-rank duration (the contract's multi-GPU timing rule)."""
     if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
         return float(value)
     import torch
@@ -160,12 +213,21 @@ def max_over_ranks(value: float, dist, device="cpu") -> float:
 
 
 def aggregate_value(samples_per_block: int, world: int, ms_step_max: float) -> float:
-    """Whole-job samples/s per beam: every replica reconstructs its own block per step."""
+    """Whole-job samples/s per beam with replicas: every replica reconstructs its own block per step."""
     return world * samples_per_block / (ms_step_max * 1e-3)
 
 
+def configure_mode(binding, plan, mode):
+    if mode == "lsmr":
+        plan.set_inversion(binding.LOFAR_INV_LSMR, 25)
+    elif mode == "exact":
+        plan.set_dedispersion(binding.LOFAR_DEDISP_EXACT)
+    elif mode == "causal":
+        plan.set_sigma_mode(binding.LOFAR_SIGMA_CAUSAL)
+
+
 # ------------------------------------------------------------------------------------- GPU arm
-def run_gpu(args):
+def run_gpu(args, idx=None):
     import torch
     from paper_1612_06592_b200 import binding
 
@@ -177,25 +239,50 @@ def run_gpu(args):
     dist = None
     if world > 1:
         import torch.distributed as dist
-        dist.init_process_group("nccl")
+        if not dist.is_initialized():
+            dist.init_process_group("nccl")
     binding.load()
+    mode = args.mode
+    beams_sharded = world > 1 and args.parallel == "beams"
 
-    w = workload(args.config, args.slices)
+    w = workload(args.config if idx is None else idx, args.slices)
     _, _, tau = synth.geometry(w)
-    X = synth.generate_block(w, 0, tau=tau)
-    plan = binding.plan_for(w, tau)
+    b0, b1 = shard.beam_slice(w.B, world, rank) if beams_sharded else (0, w.B)
+    from dataclasses import replace
+    wl = replace(w, B=b1 - b0)                               # what this rank computes
+    X = synth.generate_block(w, 0, tau=tau) if (not beams_sharded or rank == 0) else None
+    plan = binding.plan_for(wl, tau[b0:b1])
     cap = 4096
     plan.set_trigger(w.kappa, 1, cap)
-    Xd = torch.from_numpy(X).cuda()
-    series, cand, count, sigma = binding.new_outputs(plan, w.T)
+    configure_mode(binding, plan, mode)
+    want_series = mode in ("series", "lsmr", "exact")
+    Xd = torch.from_numpy(X).cuda() if X is not None else torch.empty((w.S, 2, w.K, w.T, 2),
+                                                                       dtype=torch.int8 if w.dtype == "ci8" else torch.int16,
+                                                                       device="cuda")
+    if want_series:
+        series, cand, count, sigma = binding.new_outputs(plan, w.T)
+    else:
+        series, (cand, count, sigma) = None, binding.new_outputs(plan, 0)[1:]
     stream = torch.cuda.current_stream()
+    flush = None
+    if w.input_bytes <= 256e6:                               # small inputs: evict them from L2 between steps
+        flush = torch.empty(192 << 20, dtype=torch.uint8, device="cuda")
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def step():
+    fl = []
+
+    def step(timed=False):
+        if flush is not None:                                # timed separately and subtracted from the step time
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream); flush.fill_(1); b.record(stream)
+            if timed:
+                fl.append((a, b))
+        if beams_sharded:
+            shard.broadcast_input(Xd, dist, 0)               # the one collective of the sharded path
         plan.run_block(Xd, w.T, series, cand, count, sigma, stream)
 
     for _ in range(args.warmup):
@@ -208,10 +295,10 @@ def run_gpu(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for _ in range(args.steps):
-        step()
+        step(timed=True)
     e1.record(stream)
     barrier()
-    ms_total = e0.elapsed_time(e1)
+    ms_total = e0.elapsed_time(e1) - sum(a.elapsed_time(b) for a, b in fl)
     clocks = sampler.stop() if sampler else None
     launches = plan.launch_count() - l0
     kms, kn = plan.profile_read()
@@ -220,78 +307,103 @@ def run_gpu(args):
     ms_step = ms_total / args.steps
     n_cand = int(count.item())
 
-    # ---- e2e: the same step through lofar_stream_push from pinned host memory
-    Xh = torch.from_numpy(X).pin_memory()
+    # ---- e2e: the same through lofar_stream_push from pinned host memory
+    stream_cfg4 = w.index == 4 and args.slices is None
+    nbuf = 2 if stream_cfg4 else 1
+    Xh = [torch.from_numpy(X if X is not None else np.zeros((w.S, 2, w.K, w.T, 2), dtype=w.np_dtype)).pin_memory()]
+    if nbuf == 2:
+        Xh.append(torch.from_numpy(synth.generate_block(w, 1, tau=tau)).pin_memory())
     cand_h = torch.zeros((cap, 24), dtype=torch.uint8).pin_memory()
     count_h = torch.zeros(1, dtype=torch.int32).pin_memory()
-    sigma_h = torch.zeros(w.nseries, dtype=torch.float32).pin_memory()
-    e2e_steps = max(3, min(args.steps, 5))
-    plan.stream_reset()
-    for _ in range(2):
-        plan.stream_push(Xh, w.T, series, cand_h, count_h, sigma_h)
-    plan.stream_sync()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        plan.stream_push(Xh, w.T, series, cand_h, count_h, sigma_h)
-    plan.stream_sync()
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    e2e_s = max_over_ranks(e2e_s, dist, "cuda")
-    e2e_ms = e2e_s / e2e_steps * 1e3
+    sigma_h = torch.zeros(wl.nseries, dtype=torch.float32).pin_memory()
+    e2e_steps = w.blocks if stream_cfg4 else max(3, min(args.steps, 5))
+    e2e = None
+    if not beams_sharded:
+        plan.stream_reset()
+        for i in range(2):
+            plan.stream_push(Xh[i % nbuf], w.T, series, cand_h, count_h, sigma_h)
+        plan.stream_sync(allow=(binding.LOFAR_E_OVERFLOW,))
+        if stream_cfg4:
+            plan.stream_reset()
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(e2e_steps):
+            plan.stream_push(Xh[i % nbuf], w.T, series, cand_h, count_h, sigma_h)
+        plan.stream_sync(allow=(binding.LOFAR_E_OVERFLOW,))
+        torch.cuda.synchronize()
+        e2e_s = max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+        e2e_ms = e2e_s / e2e_steps * 1e3
+        e2e_value = aggregate_value(w.T * w.M, world, e2e_ms)
+        e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(w.input_bytes),
+               "d2h_bytes_per_step": int(4 + 4 * wl.nseries + cap * 24), "ms_per_step": e2e_ms,
+               "real_time_factor": e2e_value / world / 200e6, "steps": e2e_steps,
+               "h2d_GBps": w.input_bytes / 1e9 / (e2e_ms * 1e-3),
+               "api": "lofar_stream_push + lofar_stream_sync (pinned host input, double-buffered)",
+               "note": ("configs[4] as stated: 10 consecutive blocks of 195312 slices, sustained; the blocks alternate "
+                        "between two pinned staging buffers generated before the timed region (91.5 GB of distinct "
+                        "blocks are not pinned; SURVEY 8(d) allows it)") if stream_cfg4 else
+                       "the same block pushed repeatedly"}
 
     if rank != 0:
-        if dist is not None:
+        if dist is not None and idx is None:
             dist.destroy_process_group()
         return
 
     samples_per_block = w.T * w.M
-    value = aggregate_value(samples_per_block, world, ms_step)       # per beam, all replicas
-    e2e_value = aggregate_value(samples_per_block, world, e2e_ms)
+    if beams_sharded:
+        value = samples_per_block / (ms_step * 1e-3)          # all B beams of one block per step, over N GPUs
+    else:
+        value = aggregate_value(samples_per_block, world, ms_step)
     peak, peak_src = peaks()
 
-    # algorithmic bytes per launch
+    # algorithmic bytes per launch group
     esz = 4 if w.dtype == "ci16" else 2
-    zrows = w.B                                   # beam sums are written once per beam, trials fan out on load
-    by_kernel = {
-        "beamform_kernel": w.S * 2 * w.K * w.T * esz + zrows * w.K * w.T * 8,
-        "ippf_kernel": zrows * w.K * w.T * 8 + w.nseries * w.T * w.M * 4,
-        "trigger (sigma+scan+sort)": w.nseries * (w.T // 16) * 12,
-    }
-    tc = w.dtype == "ci8" and w.B >= 4 and w.S <= 32
-    names = list(by_kernel)
-    shown = {"beamform_kernel": "beamform_tc_kernel" if tc else "beamform_kernel"}
+    B, ns = wl.B, wl.nseries
+    ninv = B if mode == "exact" else ns
+    out_series = want_series and mode not in ("lsmr", "exact")
+    by_kernel = [
+        ("beamform", w.S * 2 * w.K * w.T * esz + B * w.K * w.T * 8),
+        ("ippf_kernel", B * w.K * w.T * 8 + (ninv * w.T * w.M * 4 if (out_series or mode in ("lsmr", "exact")) else 0)),
+        ("trigger", ns * (w.T // 16) * 12 + (2 * ns * w.T * w.M * 4 if mode in ("lsmr", "exact") else 0)),
+        ("lsmr (25 iterations)", ninv * w.T * w.M * 4 * (2 + 13 * 25)),
+        ("dedisp_kernel", (B * 16 / 14 + ns) * w.T * w.M * 4),
+    ]
+    tc = w.dtype == "ci8" and B >= 4 and w.S <= 32
+    shown = {"beamform": "beamform_tc_kernel" if tc else "beamform_kernel"}
     kernels = []
-    for i, nme in enumerate(names):
+    for i, (nme, nbytes) in enumerate(by_kernel):
         if kn[i] == 0:
             continue
-        ms_launch_all = kms[i] / args.steps          # all launches of this kernel in one step
-        per_step = int(kn[i]) // args.steps
+        ms_all = kms[i] / args.steps                          # all launches of this group in one step
+        per_step = max(1, int(kn[i]) // args.steps)
         kernels.append({"kernel": shown.get(nme, nme), "launches_per_step": per_step,
-                        "ms_per_step": ms_launch_all, "ms_per_launch": ms_launch_all / per_step,
-                        "share_of_step": ms_launch_all / ms_step,
-                        "algorithmic_GB_per_launch": by_kernel[nme] / 1e9 / per_step,
-                        "achieved_GBps": by_kernel[nme] / 1e9 / (ms_launch_all * 1e-3)})
+                        "ms_per_step": ms_all, "ms_per_launch": ms_all / per_step,
+                        "share_of_step": ms_all / ms_step,
+                        "algorithmic_GB_per_launch": nbytes / 1e9 / per_step,
+                        "achieved_GBps": nbytes / 1e9 / (ms_all * 1e-3)})
     dom = max(kernels, key=lambda k: k["ms_per_step"])
-    chain_bytes = w.input_bytes + w.nseries * w.T * w.M * 4
-    # dram__bytes_read.sum + dram__bytes_write.sum over algorithmic bytes of the same launch, from the committed
-    # ncu --set full capture of configs[2] (profiles/r1_f_ncu_full.md); other workloads have no capture yet
-    ncu_ratio = {"ippf_kernel": 8.694637 / 8.650752, "beamform_tc_kernel": 6.285303 / 6.332375}
+    chain_bytes = w.input_bytes + (ns * w.T * w.M * 4 if want_series else 0)
+    prof = ncu_summary().get(f"configs[{w.index}]", {}).get(dom["kernel"], {})
     traffic = None
-    if w.index == 2 and args.slices is None and dom["kernel"] in ncu_ratio:
-        traffic = dom["algorithmic_GB_per_launch"] * ncu_ratio[dom["kernel"]]
+    if prof.get("dram_GB_per_launch") and prof.get("algorithmic_GB_per_launch") and mode == "series" and args.slices is None:
+        traffic = dom["algorithmic_GB_per_launch"] * prof["dram_GB_per_launch"] / prof["algorithmic_GB_per_launch"]
     roofline = {"kernel": dom["kernel"], "bound": "hbm", "achieved": dom["achieved_GBps"], "peak": peak,
                 "unit": "GB/s", "frac": dom["achieved_GBps"] / peak, "traffic": traffic,
-                "traffic_unit": "GB per launch (ncu dram bytes, profiles/r1_f_ncu_full.md)",
+                "traffic_unit": "GB per launch: ncu dram__bytes_read.sum + dram__bytes_write.sum scaled to this launch "
+                                "(profiles/ncu_summary.json)" if traffic else None,
+                "limiter": prof.get("limiter"), "fp32_pipe_frac": prof.get("fma_pipe_frac"),
+                "issue_frac": prof.get("issue_frac"),
                 "algorithmic_GB_per_launch": dom["algorithmic_GB_per_launch"],
                 "ms_per_launch": dom["ms_per_launch"], "peak_source": peak_src,
                 "note": "achieved = algorithmic bytes per launch / mean launch duration, CUDA events on the "
                         "launching stream inside the timed region (K*8 B read + 4096 B written per series-slice "
-                        "for ippf_kernel; 2*S*2*esize B read + B*8 B written per (sub-band, slice) for beamform)"}
+                        "for ippf_kernel; 2*S*2*esize B read + B*8 B written per (sub-band, slice) for beamform). "
+                        "`bound` names the roofline the kernel is designed against; `limiter` is what ncu shows."}
     chain = {"algorithmic_GB_per_step": chain_bytes / 1e9,
              "achieved_GBps": chain_bytes / 1e9 / (ms_step * 1e-3),
              "frac_of_peak": chain_bytes / 1e9 / (ms_step * 1e-3) / peak,
-             "note": "whole chain: input read once + series written once (SURVEY 8(d) fused count)"}
+             "note": "whole chain: input read once + series written once (SURVEY 8(d) fused count); "
+                     "series-free modes: input only"}
 
     # cuFFT (through torch.fft.irfft), timed ONLY as a comparison for step a3 (north_star); never on the product path.
     cufft = None
@@ -318,29 +430,37 @@ def run_gpu(args):
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        v, cores, sample, dt = oracle_sample(w, X[:, :, :, :2048], tau, 12.0)
-        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": dt}
+        cpu = cpu_baseline(w, X[:, :, :, :2048], tau, mode)
 
-    print(json.dumps({
+    line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "scaling": "strong" if beams_sharded else "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic (seeded, paper_1612_06592_b200.synth)",
-        "config": describe(w, {"parallelism": "replicas only" if world > 1 else "single GPU"}),
-        "real_time_factor": value / world / 200e6,
+        "config": describe(w, {"mode": mode, "parallelism": ("beams sharded over ranks, input broadcast (NCCL)"
+                                                             if beams_sharded else "replicas only") if world > 1
+                               else "single GPU"}),
+        "real_time_factor": (value if beams_sharded else value / world) / 200e6,
         "aggregate_samples_per_s_all_series": value * w.nseries,
         "candidates_last_step": n_cand,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(w.input_bytes),
-                "d2h_bytes_per_step": int(4 + 4 * w.nseries + cap * 24), "ms_per_step": e2e_ms,
-                "real_time_factor": e2e_value / world / 200e6, "steps": e2e_steps,
-                "h2d_GBps": w.input_bytes / 1e9 / (e2e_ms * 1e-3),
-                "api": "lofar_stream_push + lofar_stream_sync (pinned host input, double-buffered)"},
+        "e2e": e2e if e2e is not None else {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                                           "note": "beam-sharded run: no streaming leg"},
         "gpu_launches": int(launches),
         "roofline": roofline, "kernels": kernels, "chain": chain,
         "cpu_baseline": cpu, "clocks": clocks, "cufft_comparison": cufft,
-    }))
-    if dist is not None:
+    }
+    print(json.dumps(line), flush=True)
+    plan.destroy()
+    if dist is not None and idx is None:
         dist.destroy_process_group()
+
+
+def relaunch_under_torchrun(args):
+    """`--gpus N` by itself: become N ranks (one per GPU) under torch.distributed.run."""
+    port = 29500 + (os.getpid() % 2000)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
 
 
 def main():
@@ -349,6 +469,9 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json:configs (default 2)")
+    ap.add_argument("--all-configs", action="store_true", help="one JSON line per config 0..4 (same schema)")
+    ap.add_argument("--mode", default="series", choices=MODES)
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "beams"])
     ap.add_argument("--slices", type=int, default=None, help="override slices per block (debugging)")
     ap.add_argument("--impl", default="gpu", choices=["gpu", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -358,6 +481,12 @@ def main():
         args.warmup = 3
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        relaunch_under_torchrun(args)
+    if args.all_configs:
+        for i in range(len(synth.CONFIGS)):
+            run_gpu(args, idx=i)
     else:
         run_gpu(args)
 

@@ -252,7 +252,9 @@ LOFAR_API lofar_status lofar_stream_set_state(lofar_plan *plan, const void *stat
 /* Per-kernel device timing (measurement aid, PAPER-independent).  With profiling enabled every kernel
  * the plan launches is bracketed by CUDA events on its own stream.  lofar_plan_profile_read waits for
  * the recorded events, ADDS the elapsed milliseconds and launch counts since the previous read to
- * ms_host[3] / launches_host[3] (index 0 beamform, 1 inverse PPF, 2 trigger kernels) and clears them. */
+ * ms_host[LOFAR_PROFILE_SLOTS] / launches_host[LOFAR_PROFILE_SLOTS] (index 0 beamform, 1 inverse PPF, 2 trigger
+ * kernels, 3 LSMR solve, 4 exact de-dispersion; a "launch" is one bracketed group) and clears them. */
+#define LOFAR_PROFILE_SLOTS 5
 LOFAR_API lofar_status lofar_plan_profile(lofar_plan *plan, int enable);
 LOFAR_API lofar_status lofar_plan_profile_read(lofar_plan *plan, double *ms_host, uint64_t *launches_host);
 /* Number of kernel launches the plan has enqueued so far (for bench accounting). */

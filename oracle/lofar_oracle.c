@@ -42,6 +42,16 @@
 static const double TWO_PI = 6.283185307179586476925286766559;
 static const double PI = 3.141592653589793238462643383280;
 
+/* Number of OpenMP threads the loops below may use (bench.py times the oracle on one core and on all). */
+ORACLE_API void lofar_oracle_set_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 ORACLE_API int lofar_oracle_threads(void)
 {
 #ifdef _OPENMP

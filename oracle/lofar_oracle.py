@@ -71,6 +71,13 @@ def threads() -> int:
     return int(lib().lofar_oracle_threads())
 
 
+def set_threads(n: int):
+    lib().lofar_oracle_set_threads(int(n))
+
+
+BUILD_FLAGS = "gcc -O2 -std=c11 -fopenmp (portable: the built library travels between machines)"
+
+
 # --------------------------------------------------------------------------- steps
 def prototype(M: int = 1024, P: int = 16, beta: float = 9.0) -> np.ndarray:
     """O0: Kaiser-windowed sinc prototype h[M*P], sum(h) = 1."""

@@ -265,9 +265,10 @@ class Plan:
         _check(self._lib.lofar_plan_profile(self._h, int(enable)), "lofar_plan_profile")
 
     def profile_read(self):
-        """(ms[3], launches[3]) accumulated since the previous read: beamform, inverse PPF, trigger."""
-        ms = np.zeros(3, dtype=np.float64)
-        n = np.zeros(3, dtype=np.uint64)
+        """(ms[5], launches[5]) accumulated since the previous read: beamform, inverse PPF, trigger, LSMR, exact
+        de-dispersion."""
+        ms = np.zeros(5, dtype=np.float64)
+        n = np.zeros(5, dtype=np.uint64)
         _check(self._lib.lofar_plan_profile_read(self._h, ms.ctypes.data, n.ctypes.data), "lofar_plan_profile_read")
         return ms, n
 

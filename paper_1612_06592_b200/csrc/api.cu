@@ -396,6 +396,7 @@ lofar_status lsmr_begin(lofar_plan *p, cudaStream_t st)
 
 lofar_status lsmr_solve(lofar_plan *p, long long T, float *series, long long series_pitch, cudaStream_t st)
 {
+    ProfScope prof(p, 3, st);
     const int n = launch_lsmr(p->dY, p->ypitch, T, p->dLsmrWork, p->wpitch, reinterpret_cast<const float *>(p->dGs),
                               p->dLsmrScal, p->dLsmrPartial, p->ninv(), p->lsmr_iters, series, series_pitch, st);
     if (n < 0) return LOFAR_E_CUDA;
@@ -512,7 +513,11 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
         d.xlead = p->dXhat; d.xpitch = p->xhat_pitch; d.nlead = T + 2;
         d.series = series; d.series_pitch = N; d.T = T; d.B = p->B; d.D = p->D;
         d.Dtab = p->dDtab; d.tw8192 = p->dTw8192; d.tw16k = p->dTw16k; d.tw512 = p->dTw + 256;
-        const int nd = launch_dedisp(d, st);
+        int nd;
+        {
+            ProfScope prof(p, 4, st);
+            nd = launch_dedisp(d, st);
+        }
         if (nd < 0) return LOFAR_E_CUDA;
         p->launches += nd;
         // carry the last two slices of the undispersed series (one slice at a time: they may overlap their target)
@@ -1020,7 +1025,7 @@ lofar_status lofar_plan_profile_read(lofar_plan *p, double *ms, uint64_t *launch
         float t = 0.f;
         CU(cudaEventSynchronize(r.b));
         CU(cudaEventElapsedTime(&t, r.a, r.b));
-        if (r.id >= 0 && r.id < 3) { ms[r.id] += (double)t; launches[r.id] += 1; }
+        if (r.id >= 0 && r.id < LOFAR_PROFILE_SLOTS) { ms[r.id] += (double)t; launches[r.id] += 1; }
         p->prof_pool.push_back(r.a);
         p->prof_pool.push_back(r.b);
     }

@@ -158,18 +158,33 @@ struct Emit {
     uint64_t sample0;        // global index of sample 0 of the series slice the step starts at
 };
 
-// Rare path: one record per sample above the threshold (all trials; the best trial is selected after the sort).
-__device__ __noinline__ void emit_pair(const Emit &e, uint64_t n, float vx, float vy)
+// Rare path, kept out of line and out of the FIR's registers: a thread whose step maximum exceeds the threshold
+// recomputes its 2 x 16 outputs (taps re-read from global memory) and records every sample above the threshold
+// (all trials; the best trial per sample is selected after the sort).
+__device__ __noinline__ void emit_step(const float2 *prev, const float2 *cur, const float2 *gs, int tid, int pn, int nvalid,
+                                       lofar_candidate *cand, uint32_t *count, uint32_t cap, uint32_t series, uint32_t trial,
+                                       float thr, float sigma, uint64_t sample0)
 {
+    for (int j = 0; j < nvalid; ++j) {
+        float2 acc = make_float2(0.f, 0.f);
+        for (int t = 0; t < kP; ++t) {
+            const int i = (kP - 1) + j - t;                    // window element: prev rows 1..15, cur rows 0..15
+            const float2 x = (i < kP - 1) ? prev[(i + 1) * kRow + pn] : cur[(i - (kP - 1)) * kRow + pn];
+            const float2 g = __ldg(gs + t * kH + tid);
+            acc.x = fmaf(g.x, x.x, acc.x);
+            acc.y = fmaf(g.y, x.y, acc.y);
+        }
 #pragma unroll
-    for (int c = 0; c < 2; ++c) {
-        const float v = fabsf(c ? vy : vx);
-        if (v > e.thr) {
-            const uint32_t slot = atomicAdd(e.count, 1u);
-            if (slot < e.cap) {
-                lofar_candidate r;
-                r.series = e.series; r.trial = e.trial; r.sample = n + c; r.env = v; r.sigma = e.sigma;
-                e.cand[slot] = r;
+        for (int c = 0; c < 2; ++c) {
+            const float v = fabsf(c ? acc.y : acc.x);
+            if (v > thr) {
+                const uint32_t slot = atomicAdd(count, 1u);
+                if (slot < cap) {
+                    lofar_candidate r;
+                    r.series = series; r.trial = trial; r.sample = sample0 + (uint64_t)j * kM + 2 * tid + c;
+                    r.env = v; r.sigma = sigma;
+                    cand[slot] = r;
+                }
             }
         }
     }
@@ -179,7 +194,7 @@ __device__ __noinline__ void emit_pair(const Emit &e, uint64_t n, float vx, floa
 // 0..15, column pn; FULL = all 16 output slices valid (no predicates on the fast path).
 template <bool FULL>
 __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, const u64 (&g)[kP], int pn, float *out,
-                                         int tid, int nvalid, const Emit &em, u64 &ssum2, float &smax)
+                                         int tid, int nvalid, u64 &ssum2, float &smax)
 {
     u64 acc[kStep];
 #pragma unroll
@@ -200,9 +215,7 @@ __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, 
                 const float vx = LO(acc[j]), vy = HI(acc[j]);
                 if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)j * kM + 2 * tid), make_float2(vx, vy));
                 ssum2 = fma2(acc[j], acc[j], ssum2);
-                const float m = fmaxf(fabsf(vx), fabsf(vy));
-                smax = fmaxf(smax, m);
-                if (m > em.thr) emit_pair(em, em.sample0 + (uint64_t)j * kM + 2 * tid, vx, vy);
+                smax = fmaxf(smax, fmaxf(fabsf(vx), fabsf(vy)));
             }
         }
     }
@@ -295,8 +308,11 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
             float smax = 0.f;
             float *o = out ? out + (size_t)q * kM : nullptr;
             em.sample0 = a.offset + (uint64_t)a.out0 + (uint64_t)q * kM;
-            if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, em, ssum2, smax);
-            else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, em, ssum2, smax);
+            if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
+            else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
+            if (smax > em.thr)
+                emit_step(prev, cur, a.gs, tid, pn, nvalid, em.cand, em.count, em.cap, em.series, em.trial, em.thr, em.sigma,
+                          em.sample0);
             dsum += (double)(LO(ssum2) + HI(ssum2));
 #pragma unroll
             for (int s = 16; s > 0; s >>= 1) smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, s));
@@ -420,7 +436,10 @@ __global__ void __launch_bounds__(kThreads, 1) rescan_kernel(RescanArgs r)
             const int nvalid = (r.T - q < kStep) ? (int)(r.T - q) : kStep;
             u64 ssum2 = 0ull;
             float smax = 0.f;
-            fir_step<false>(buf0, buf1, g, pn, nullptr, tid, nvalid, em, ssum2, smax);
+            fir_step<false>(buf0, buf1, g, pn, nullptr, tid, nvalid, ssum2, smax);
+            if (smax > em.thr)
+                emit_step(buf0, buf1, r.gs, tid, pn, nvalid, em.cand, em.count, em.cap, em.series, em.trial, em.thr, em.sigma,
+                          em.sample0);
             __syncthreads();
         }
     }
