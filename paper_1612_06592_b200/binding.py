@@ -59,10 +59,11 @@ def load() -> ctypes.CDLL:
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
-        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1612_06592_b200.build` "
+    path = os.environ.get("LOFAR_MOON_LIB", LIB_PATH)      # ablation builds of build.py; default: the in-tree library
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: build it with `python -m paper_1612_06592_b200.build` "
                            "(there is no CPU fallback)")
-    lib = ctypes.CDLL(LIB_PATH)
+    lib = ctypes.CDLL(path)
     c = ctypes
     vp, i, d, u32, u64 = c.c_void_p, c.c_int, c.c_double, c.c_uint32, c.c_uint64
     sig = {

@@ -2,6 +2,12 @@
 
 `python -m paper_1612_06592_b200.build [--force] [--verbose]` or `build()` from Python.
 nvcc cross-compiles without a GPU; the .so sits next to this file so that it travels with the tree.
+
+Ablation builds (the measurements DESIGN.md section 8 quotes): `--define NAME [--define NAME ...] --out PATH` compiles a
+variant with -DNAME into PATH (objects under build/<names>/); run it with LOFAR_MOON_LIB=PATH, which the binding
+honours. Switches: LOFAR_FIR_SCALAR (synthesis FIR with scalar FFMA instead of packed FFMA2), LOFAR_ABLATE_STORES
+(inverse PPF without its series stores), LOFAR_ABLATE_FIR (no FIR arithmetic), LOFAR_ABLATE_FFT (no transform
+arithmetic). Ablated variants compute wrong results by design; they exist to attribute time.
 """
 from __future__ import annotations
 
@@ -30,33 +36,37 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
+def build(force: bool = False, verbose: bool = False, defines=(), out: str | None = None) -> str:
+    if not defines and out is None and not force and not _stale():
         return LIB
-    objdir = os.path.join(HERE, "build")
+    objdir = os.path.join(HERE, "build", *(["_".join(defines)] if defines else []))
     os.makedirs(objdir, exist_ok=True)
+    lib = out or LIB
     procs = []
     objs = []
     for s in SOURCES:
         o = os.path.join(objdir, s.replace(".cu", ".o"))
         objs.append(o)
-        cmd = [NVCC, *FLAGS, "-c", os.path.join(CSRC, s), "-o", o]
+        cmd = [NVCC, *FLAGS, *[f"-D{d}" for d in defines], "-c", os.path.join(CSRC, s), "-o", o]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     failed = False
     for s, p in procs:
-        out, _ = p.communicate()
+        log, _ = p.communicate()
         if p.returncode != 0 or verbose:
-            sys.stderr.write(f"--- nvcc {s} (exit {p.returncode})\n{out}\n")
+            sys.stderr.write(f"--- nvcc {s} (exit {p.returncode})\n{log}\n")
         failed = failed or p.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed")
-    tmp = LIB + f".tmp{os.getpid()}"
+    tmp = lib + f".tmp{os.getpid()}"
     subprocess.check_call([NVCC, "-shared", "-o", tmp, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    argv = sys.argv[1:]
+    defs = [argv[i + 1] for i, a in enumerate(argv) if a == "--define"]
+    outs = [argv[i + 1] for i, a in enumerate(argv) if a == "--out"]
+    print(build(force="--force" in argv, verbose="--verbose" in argv, defines=tuple(defs), out=outs[0] if outs else None))

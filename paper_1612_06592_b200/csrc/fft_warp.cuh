@@ -65,26 +65,25 @@ __device__ __forceinline__ void idft16p(u64 *x)
     { const u64 t = cmulp(o[7], -c1, s1); x[7] = add2(e[7], t); x[15] = sub2(e[7], t); }
 }
 
-// 512-point inverse complex FFT of one slice row by one warp, in place: 512 = 16 x 32.
-//   pass A: lane j does the 16-point DFT of elements j + 32 r and writes them to 16 j + m;
-//   pass B: butterfly j (0..15) is a 32-point DFT of elements j + 16 r with twiddles exp(2 pi i j r / 512);
-//           lanes j and j + 16 share it: each does the 16-point DFT of the even / odd r, the odd lane applies
-//           W32^m, the halves are exchanged with shuffles; outputs go to j + 16 m (m < 16 low lane, m >= 16 high).
-__device__ __forceinline__ void fft512_warp(float2 *row, const float2 *stw, int lane)
+// Radix-32 pass of the 512-point inverse FFT (512 = 16 x 32) of one slice row by one warp, in place. The row holds
+// the radix-16 results at 16 j + m. Butterfly j (0..15) is a 32-point DFT of elements j + 16 r with twiddles
+// exp(2 pi i j r / 512) (TW: applied here on load; otherwise the producer of the row has applied them);
+// lanes j and j + 16 share it: each does the 16-point DFT of the even / odd r, the odd lane applies W32^m, the
+// halves are exchanged with shuffles; outputs go to j + 16 m (m < 16 low lane, m >= 16 high).
+template <bool TW>
+__device__ __forceinline__ void fft512_pass_b(float2 *row, const float2 *stw, int lane)
 {
     u64 x[16];
+    if (TW) {
+        const float2 *T = stw + 256 + lane;      // T[32 r' + lane] = exp(2 pi i j (hh + 2 r') / 512)
 #pragma unroll
-    for (int r = 0; r < 16; ++r) x[r] = lds64(row + pad(lane + 32 * r));
-    idft16p(x);
-    __syncwarp();
+        for (int r = 0; r < 16; ++r) {
+            const float2 t = T[32 * r];
+            x[r] = cmulp(lds64(row + pad(lane + 32 * r)), t.x, t.y);
+        }
+    } else {
 #pragma unroll
-    for (int m = 0; m < 16; ++m) sts64(row + pad(16 * lane + m), x[m]);
-    __syncwarp();
-    const float2 *T = stw + 256 + lane;          // T[32 r' + lane] = exp(2 pi i j (hh + 2 r') / 512)
-#pragma unroll
-    for (int r = 0; r < 16; ++r) {
-        const float2 t = T[32 * r];
-        x[r] = cmulp(lds64(row + pad(lane + 32 * r)), t.x, t.y);
+        for (int r = 0; r < 16; ++r) x[r] = lds64(row + pad(lane + 32 * r));
     }
     idft16p(x);
     const bool hi = lane >= 16;
@@ -115,6 +114,22 @@ __device__ __forceinline__ void fft512_warp(float2 *row, const float2 *stw, int 
 #pragma unroll
     for (int m = 0; m < 16; ++m) sts64(row + pad(base + 16 * m), x[m]);
     __syncwarp();
+}
+
+// 512-point inverse complex FFT of one slice row by one warp, in place:
+//   pass A: lane j does the 16-point DFT of elements j + 32 r and writes them to 16 j + m;
+//   pass B: fft512_pass_b with the twiddles applied on load.
+__device__ __forceinline__ void fft512_warp(float2 *row, const float2 *stw, int lane)
+{
+    u64 x[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) x[r] = lds64(row + pad(lane + 32 * r));
+    idft16p(x);
+    __syncwarp();
+#pragma unroll
+    for (int m = 0; m < 16; ++m) sts64(row + pad(16 * lane + m), x[m]);
+    __syncwarp();
+    fft512_pass_b<true>(row, stw, lane);
 }
 
 }  // namespace lofar

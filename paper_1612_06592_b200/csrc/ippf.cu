@@ -29,7 +29,7 @@ namespace {
 constexpr int kThreads = 512;
 constexpr int kTwCount = 256 + 512;        // w1024[256], TB[32][16] = exp(2 pi i j r / 512)
 constexpr int kStageF2 = kH * kStep;       // stage: up to 512 rows x 16 slices of float2 = 64 KB
-constexpr size_t kSmemBytes = (size_t)(2 * kStep * kRow + kStageF2 + kTwCount) * sizeof(float2) + 256;
+constexpr size_t kSmemBytes = (size_t)(2 * kStep * kRow + kStageF2 + kTwCount + kH) * sizeof(float2) + 256;
 
 // ---- mbarrier + bulk asynchronous copy (TMA unit, SASS UBLKCP / SYNCS) ------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -61,7 +61,7 @@ struct Ctx {
     int K, k0, bulk_rows, tiled;
 };
 
-// Brings the K rows x 16 slices of the step starting at slice q into the stage ([K][16] float2).
+// Brings the K rows x 16 slices of the step starting at slice q into rows k0 .. k0 + K - 1 of the stage (`stage` points at row k0).
 // Returns true if the copy is asynchronous (completion on the mbarrier), false if the threads stored it.
 __device__ __forceinline__ bool stage_fill(const Ctx &c, long long q, float2 *stage, uint32_t bar, int tid)
 {
@@ -93,58 +93,81 @@ __device__ __forceinline__ bool stage_fill(const Ctx &c, long long q, float2 *st
     return false;
 }
 
-__device__ __forceinline__ float4 rotate2(float4 v, float2 f)
+// ---- pass A: pair pre-pass fused with the radix-16 pass of the 512-point transform ---------------------
+// The stage is indexed by the absolute bin: row m holds the 16 slices of bin m; the rows of unselected bins are
+// zeroed once per CTA (reading A10) and the copies only ever write rows k0 .. k0 + K - 1, so the transform reads
+// it without bounds tests. The STEC trial phasor (a2, sph[m]) multiplies a beam sum as it enters the transform.
+template <bool PH>
+__device__ __forceinline__ u64 ldz(const float2 *p, const float2 *ph)
 {
-    return make_float4(f.x * v.x - f.y * v.y, f.x * v.y + f.y * v.x, f.x * v.z - f.y * v.w, f.x * v.w + f.y * v.z);
+    const u64 v = lds64(p);
+    if (!PH) return v;
+    const float2 f = *ph;
+    return cmulp(v, f.x, f.y);
 }
 
-// Pre-pass of the 16 staged slices into dst[16][kRow] (packed half-spectrum V, slice-major).
-// Thread unit i covers the conjugate pair m = (tid>>3) + 64 i (m = 0: bins 0 and 256) and slices 2tp, 2tp+1.
+// One conjugate pair: a = Y[m], b = Y[512-m], w = exp(2 pi i m / 1024):
 //   P = a + conj(b), D = a - conj(b), U' = (Im(wD), Re(wD));  V[m] = (P.x - U'.x, P.y + U'.y),
-//   V[512-m] = (P.x + U'.x, U'.y - P.y)            (fft_math.cuh: prepass_pair, restated for packed ops)
-__device__ __forceinline__ void prepass(const Ctx &c, const float2 *stage, float2 *dst, const float2 *stw, int tid)
+//   V[512-m] = (P.x + U'.x, U'.y - P.y)                                 (fft_math.cuh)
+__device__ __forceinline__ void vpair(u64 a, u64 b, float2 w, u64 &vm, u64 &vmir)
 {
-    const int tp = tid & 7, m0 = tid >> 3;
-    float2 *r0 = dst + 2 * tp * kRow, *r1 = r0 + kRow;
     const u64 pm = PK(1.f, -1.f), mp = PK(-1.f, 1.f);
-    const float4 *st4 = reinterpret_cast<const float4 *>(stage) + tp;      // + 8 float4 per row
+    const u64 P = fma2(b, pm, a), D = fma2(b, mp, a);
+    const float dx = LO(D), dy = HI(D);
+    const u64 U = PK(fmaf(w.x, dy, w.y * dx), fmaf(w.x, dx, -w.y * dy));
+    vm = fma2(U, mp, P);
+    vmir = fma2(P, pm, U);
+}
+
+// All 512 threads, one step: thread (j, t) -- j = residue of the bin index mod 32, t = slice of the step -- builds
+// V[j + 32 r], r = 0..15, of its slice straight from the stage ([512][16], so the 16 slices of a half-warp read one
+// 128-byte line), does the 16-point DFT over r, applies the radix-32 twiddles exp(2 pi i j m / 512) and stores
+// the result slice-major at dst[t][pad(16 j + m)]. The mirror of bin j + 32 r is bin (32 - j) + 32 (15 - r): a
+// warp holds j in its low and 32 - j in its high half, each thread forms the pairs r = 0..7 and hands the
+// mirrored values to its partner lane (shuffle); warp 0 holds the two self-paired residues j = 0 and j = 16.
+template <bool PH>
+__device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, float2 *dst, const float2 *stw, int tid)
+{
+    const int warp = tid >> 5, lane = tid & 31, half = lane >> 4, t = lane & 15;
+    constexpr int R = 32 * kStep;                  // stage elements between bins m and m + 32
+    u64 x[16];
+    int j;
+    if (warp == 0) {
+        const float2 *s0 = stage + t;
+        if (half == 0) {
+            j = 0;
+            const u64 y0 = ldz<PH>(s0, sph), y256 = ldz<PH>(s0 + 256 * kStep, sph + 256);
+            x[0] = PK(LO(y0), LO(y0));                              // prepass_dc
+            x[8] = PK(2.0f * LO(y256), -2.0f * HI(y256));           // prepass_quarter
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int m = m0 + 64 * i;
-        const unsigned ja = (unsigned)(m - c.k0), jb = (unsigned)((m == 0 ? 256 : 512 - m) - c.k0);
-        float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
-        if (ja < (unsigned)c.K) a = st4[ja * 8];
-        if (jb < (unsigned)c.K) b = st4[jb * 8];
-        if (c.ph) {
-            // STEC trial fan-out (a2): the trial's phasor multiplies the beam sums as they enter the transform
-            if (ja < (unsigned)c.K) a = rotate2(a, __ldg(c.ph + ja));
-            if (jb < (unsigned)c.K) b = rotate2(b, __ldg(c.ph + jb));
-        }
-        if (m == 0) {
-            r0[pad(0)] = prepass_dc(make_float2(a.x, a.y));
-            r1[pad(0)] = prepass_dc(make_float2(a.z, a.w));
-            r0[pad(256)] = prepass_quarter(make_float2(b.x, b.y));
-            r1[pad(256)] = prepass_quarter(make_float2(b.z, b.w));
+            for (int r = 1; r < 8; ++r)
+                vpair(ldz<PH>(s0 + r * R, sph + 32 * r), ldz<PH>(s0 + (16 - r) * R, sph + 512 - 32 * r), stw[32 * r], x[r],
+                      x[16 - r]);
         } else {
-            const float2 w = stw[m];
-            const int im = pad(m), imir = pad(512 - m);
-            {
-                const u64 A = PK(a.x, a.y), B = PK(b.x, b.y);
-                const u64 P = fma2(B, pm, A), D = fma2(B, mp, A);
-                const float dx = LO(D), dy = HI(D);
-                const u64 U = PK(fmaf(w.x, dy, w.y * dx), fmaf(w.x, dx, -w.y * dy));
-                sts64(r0 + im, fma2(U, mp, P));
-                sts64(r0 + imir, fma2(P, pm, U));
-            }
-            {
-                const u64 A = PK(a.z, a.w), B = PK(b.z, b.w);
-                const u64 P = fma2(B, pm, A), D = fma2(B, mp, A);
-                const float dx = LO(D), dy = HI(D);
-                const u64 U = PK(fmaf(w.x, dy, w.y * dx), fmaf(w.x, dx, -w.y * dy));
-                sts64(r1 + im, fma2(U, mp, P));
-                sts64(r1 + imir, fma2(P, pm, U));
-            }
+            j = 16;
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+                vpair(ldz<PH>(s0 + 16 * kStep + r * R, sph + 16 + 32 * r),
+                      ldz<PH>(s0 + 16 * kStep + (15 - r) * R, sph + 496 - 32 * r), stw[16 + 32 * r], x[r], x[15 - r]);
         }
+    } else {
+        j = half ? 32 - warp : warp;
+        const float2 *sa = stage + j * kStep + t, *sb = stage + (512 - j) * kStep + t;
+        const float2 *pa = sph + j, *pb = sph + 512 - j, *wj = stw + j;
+        u64 give[8];
+#pragma unroll
+        for (int r = 0; r < 8; ++r) vpair(ldz<PH>(sa + r * R, pa + 32 * r), ldz<PH>(sb - r * R, pb - 32 * r), wj[32 * r], x[r], give[r]);
+#pragma unroll
+        for (int r = 0; r < 8; ++r) x[15 - r] = __shfl_xor_sync(0xffffffffu, give[r], 16);
+    }
+    idft16p(x);
+    const float2 *T = stw + 256 + 16 * j;          // T[m] = exp(2 pi i j m / 512)
+    float2 *row = dst + t * kRow + 17 * j;         // pad(16 j + m) = 17 j + m
+    sts64(row, x[0]);
+#pragma unroll
+    for (int m = 1; m < 16; ++m) {
+        const float2 f = T[m];
+        sts64(row + m, cmulp(x[m], f.x, f.y));
     }
 }
 
@@ -190,6 +213,16 @@ __device__ __noinline__ void emit_step(const float2 *prev, const float2 *cur, co
     }
 }
 
+// One tap of the FIR on a residue pair: packed FFMA2 (half the issue slots) or, with -DLOFAR_FIR_SCALAR, two FFMA.
+__device__ __forceinline__ u64 fir_fma(u64 g, u64 x, u64 acc)
+{
+#ifdef LOFAR_FIR_SCALAR
+    return PK(fmaf(LO(g), LO(x), LO(acc)), fmaf(HI(g), HI(x), HI(acc)));
+#else
+    return fma2(g, x, acc);
+#endif
+}
+
 // Synthesis FIR of one step: out[j] = sum_t g[t] * win[15 + j - t], j = 0..15, window = prev rows 1..15 + cur rows
 // 0..15, column pn; FULL = all 16 output slices valid (no predicates on the fast path).
 template <bool FULL>
@@ -205,7 +238,7 @@ __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, 
 #pragma unroll
         for (int t = 0; t < kP; ++t) {
             const int j = i - (kP - 1) + t;
-            if (j >= 0 && j < kStep) acc[j] = fma2(g[t], x, acc[j]);
+            if (j >= 0 && j < kStep) acc[j] = fir_fma(g[t], x, acc[j]);
         }
         // output slice j = i - 15 is complete once window element i has been applied: store it now so
         // that the 64 KB of stores per step are spread over the second half of the FIR
@@ -213,7 +246,9 @@ __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, 
             const int j = i - (kP - 1);
             if (FULL || j < nvalid) {
                 const float vx = LO(acc[j]), vy = HI(acc[j]);
+#ifndef LOFAR_ABLATE_STORES
                 if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)j * kM + 2 * tid), make_float2(vx, vy));
+#endif
                 ssum2 = fma2(acc[j], acc[j], ssum2);
                 smax = fmaxf(smax, fmaxf(fabsf(vx), fabsf(vy)));
             }
@@ -224,11 +259,12 @@ __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, 
 __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float2 *stage = reinterpret_cast<float2 *>(smem_raw);          // [K][16], 128-byte aligned for the bulk copies
+    float2 *stage = reinterpret_cast<float2 *>(smem_raw);          // [512][16] by bin, 128-byte aligned for the bulk copies
     float2 *buf0 = stage + kStageF2;
     float2 *buf1 = buf0 + kStep * kRow;
     float2 *stw = buf1 + kStep * kRow;                             // [kTwCount]
-    float *sred = reinterpret_cast<float *>(stw + kTwCount);       // 16 floats, 16 doubles, the mbarrier
+    float2 *sph = stw + kTwCount;                                  // [K] phasors of this series' STEC trial (a2)
+    float *sred = reinterpret_cast<float *>(sph + kH);             // 16 floats, 16 doubles, the mbarrier
     double *sdred = reinterpret_cast<double *>(sred + 16);
     const uint32_t bar = smem_u32(sdred + 16);
 
@@ -251,6 +287,13 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = tid; i < kTwCount; i += kThreads) stw[i] = a.tw[i];
+    for (int i = tid; i < kStageF2; i += kThreads) stage[i] = make_float2(0.f, 0.f);   // unselected bins stay zero
+    if (c.ph) {
+        sph[tid] = make_float2(1.f, 0.f);
+        __syncthreads();
+        for (int i = tid; i < a.K; i += kThreads) sph[a.k0 + i] = c.ph[i];
+    }
+    float2 *stage_k = stage + a.k0 * kStep;      // the copies write rows k0 .. k0 + K - 1
     u64 g[kP];                                   // the 16 tap pairs of residues 2 tid, 2 tid + 1, for the whole span
 #pragma unroll
     for (int t = 0; t < kP; ++t) { const float2 v = __ldg(a.gs + t * kH + tid); g[t] = PK(v.x, v.y); }
@@ -268,7 +311,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     // the first step of a span that starts inside the block is a warm-up: transform the 16 slices before it
     const long long q_first = span == 0 ? qs : qs - kStep;
     uint32_t phase = 0;
-    bool async = stage_fill(c, q_first, stage, bar, tid);
+    bool async = stage_fill(c, q_first, stage_k, bar, tid);
 
     float *out = a.series ? a.series + (size_t)series * a.series_pitch + a.out0 : nullptr;
     float *yout = a.yout ? a.yout + (size_t)series * a.yout_pitch + a.out0 : nullptr;
@@ -282,10 +325,15 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     for (long long q = q_first; q < qe; q += kStep) {
         if (async) { while (!mbar_try_wait(bar, phase)) {} phase ^= 1; }
         else __syncthreads();
-        prepass(c, stage, cur, stw, tid);
-        __syncthreads();                         // cur complete, stage free
-        if (q + kStep < qe) async = stage_fill(c, q + kStep, stage, bar, tid);   // flies during FFT + FIR
-        fft512_warp(cur + warp * kRow, stw, lane);
+#ifndef LOFAR_ABLATE_FFT
+        if (c.ph) pass_a<true>(stage, sph, cur, stw, tid);
+        else pass_a<false>(stage, sph, cur, stw, tid);
+#endif
+        __syncthreads();                         // radix-16 results of all 16 slices in cur, stage free
+        if (q + kStep < qe) async = stage_fill(c, q + kStep, stage_k, bar, tid);   // flies during pass B + FIR
+#ifndef LOFAR_ABLATE_FFT
+        fft512_pass_b<false>(cur + warp * kRow, stw, lane);
+#endif
         __syncthreads();
 
         if (q >= qs && yout) {
@@ -308,8 +356,10 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
             float smax = 0.f;
             float *o = out ? out + (size_t)q * kM : nullptr;
             em.sample0 = a.offset + (uint64_t)a.out0 + (uint64_t)q * kM;
+#ifndef LOFAR_ABLATE_FIR
             if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
             else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
+#endif
             if (smax > em.thr)
                 emit_step(prev, cur, a.gs, tid, pn, nvalid, em.cand, em.count, em.cap, em.series, em.trial, em.thr, em.sigma,
                           em.sample0);
@@ -390,10 +440,14 @@ __global__ void __launch_bounds__(kThreads, 1) rescan_kernel(RescanArgs r)
     float2 *buf0 = stage + kStageF2;
     float2 *buf1 = buf0 + kStep * kRow;
     float2 *stw = buf1 + kStep * kRow;
+    float2 *sph = stw + kTwCount;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t total = *r.nitems < r.items_cap ? *r.nitems : r.items_cap;
     if (blockIdx.x >= total) return;
     for (int i = tid; i < kTwCount; i += kThreads) stw[i] = r.tw[i];
+    for (int i = tid; i < kStageF2; i += kThreads) stage[i] = make_float2(0.f, 0.f);
+    sph[tid] = make_float2(1.f, 0.f);
+    float2 *stage_k = stage + r.k0 * kStep;
     u64 g[kP];
 #pragma unroll
     for (int t = 0; t < kP; ++t) { const float2 v = __ldg(r.gs + t * kH + tid); g[t] = PK(v.x, v.y); }
@@ -407,27 +461,28 @@ __global__ void __launch_bounds__(kThreads, 1) rescan_kernel(RescanArgs r)
             const int series = beam * r.D + d;
             const float sig = r.sigma[series], thr = r.kappa * sig;
             if (r.chunkmax[(size_t)series * r.chunkmax_pitch + r.items[it].y] < thr * 0.99999f) continue;
-            Ctx c;
-            c.Zs = nullptr; c.ph = r.D > 1 ? r.Dph + (size_t)d * r.K : nullptr;
-            c.zpitch = 0; c.nc = r.T; c.K = r.K; c.k0 = r.k0; c.bulk_rows = 0; c.tiled = 0;
+            if (r.D > 1)                               // this trial's phasors (read by pass_a after the next barrier)
+                for (int i = tid; i < r.K; i += kThreads) sph[r.k0 + i] = r.Dph[(size_t)d * r.K + i];
             if (q == 0) {
                 const float *h = r.hist0 + (size_t)series * (kP - 1) * kM;
 #pragma unroll
                 for (int i = 0; i < kP - 1; ++i)
                     buf0[(i + 1) * kRow + pn] = *reinterpret_cast<const float2 *>(h + (size_t)i * kM + 2 * tid);
             } else {
-                stage_from_x(r, beam, q - kStep, stage, tid);
+                stage_from_x(r, beam, q - kStep, stage_k, tid);
                 __syncthreads();
-                prepass(c, stage, buf0, stw, tid);
+                if (r.D > 1) pass_a<true>(stage, sph, buf0, stw, tid);
+                else pass_a<false>(stage, sph, buf0, stw, tid);
                 __syncthreads();
-                fft512_warp(buf0 + warp * kRow, stw, lane);
+                fft512_pass_b<false>(buf0 + warp * kRow, stw, lane);
             }
             __syncthreads();
-            stage_from_x(r, beam, q, stage, tid);
+            stage_from_x(r, beam, q, stage_k, tid);
             __syncthreads();
-            prepass(c, stage, buf1, stw, tid);
+            if (r.D > 1) pass_a<true>(stage, sph, buf1, stw, tid);
+            else pass_a<false>(stage, sph, buf1, stw, tid);
             __syncthreads();
-            fft512_warp(buf1 + warp * kRow, stw, lane);
+            fft512_pass_b<false>(buf1 + warp * kRow, stw, lane);
             __syncthreads();
             Emit em;
             em.cand = r.cand; em.count = r.count; em.cap = r.cap;
