@@ -255,6 +255,10 @@ def run_gpu(args, idx=None):
     cap = 4096
     plan.set_trigger(w.kappa, 1, cap)
     configure_mode(binding, plan, mode)
+    if args.overlap:
+        plan.set_overlap(1, args.overlap_chunk)              # two-lane pipeline (measured slower; off by default)
+    if args.scratch_mb:
+        plan.set_scratch_limit(args.scratch_mb << 20)        # e.g. an L2-sized beam-sum chunk
     want_series = mode in ("series", "lsmr", "exact")
     Xd = torch.from_numpy(X).cuda() if X is not None else torch.empty((w.S, 2, w.K, w.T, 2),
                                                                        dtype=torch.int8 if w.dtype == "ci8" else torch.int16,
@@ -437,7 +441,10 @@ def run_gpu(args, idx=None):
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "strong" if beams_sharded else "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic (seeded, paper_1612_06592_b200.synth)",
-        "config": describe(w, {"mode": mode, "parallelism": ("beams sharded over ranks, input broadcast (NCCL)"
+        "config": describe(w, {"mode": mode, "pipeline": ("two-lane (lofar_plan_set_overlap 1)" if args.overlap else "serial"),
+                               "chunks": [list(c) for c in plan.chunks(w.T)][:3] + ["..."] if len(plan.chunks(w.T)) > 3
+                               else [list(c) for c in plan.chunks(w.T)],
+                               "parallelism": ("beams sharded over ranks, input broadcast (NCCL)"
                                                              if beams_sharded else "replicas only") if world > 1
                                else "single GPU"}),
         "real_time_factor": (value if beams_sharded else value / world) / 200e6,
@@ -475,6 +482,10 @@ def main():
     ap.add_argument("--slices", type=int, default=None, help="override slices per block (debugging)")
     ap.add_argument("--impl", default="gpu", choices=["gpu", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--overlap", action="store_true",
+                    help="lofar_plan_set_overlap(1): beamformer of chunk c+1 beside the inverse PPF of chunk c")
+    ap.add_argument("--overlap-chunk", type=int, default=0, help="slices per pipeline chunk (0 = library default)")
+    ap.add_argument("--scratch-mb", type=int, default=0, help="lofar_plan_set_scratch_limit in MiB (0 = default 4 GiB)")
     ap.add_argument("--compare-cufft", action="store_true", help="also time cuFFT C2R (via torch) as a comparison for a3")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "gpu":

@@ -164,14 +164,31 @@ LOFAR_API lofar_status lofar_plan_workspace_bytes(lofar_plan *plan, size_t *byte
  * only memory the plan takes elsewhere is 256 bytes of pinned HOST memory for streaming counts. */
 LOFAR_API lofar_status lofar_plan_set_allocator(lofar_plan *plan, void *(*alloc)(size_t, void *),
                                                 void (*free_)(void *, void *), void *ctx);
-/* Upper bound in bytes for the beam-sum scratch of one time chunk (default 4 GiB).  A block longer
+/* Upper bound in bytes for the beam-sum scratch (default 4 GiB; all slots together).  A block longer
  * than the chunk is processed chunk by chunk, history handed over on the device. */
 LOFAR_API lofar_status lofar_plan_set_scratch_limit(lofar_plan *plan, size_t bytes);
+/* Two-lane block pipeline of lofar_run_block / lofar_stream_push (step a6 applied inside a block: the "CUDA
+ * streams" of BASELINE.json:north_star (e)).  mode 0 (default): both kernels of every chunk run back to back on
+ * the caller's stream.  mode 1: when the tensor-core beamformer is in use (int8 input, >= 4 beams) and the
+ * block is longer than one chunk, the block is cut into chunks of `chunk_slices` (0 = 8192; never more than
+ * half the scratch limit), the beamformer of chunk c+1 runs on a low-priority plan-owned stream while the
+ * inverse PPF of chunk c runs on a high-priority one, on alternating scratch slots; the inverse PPF is planned
+ * for 16 SMs fewer (one wave), which the beamformer uses.  The caller's stream forks into the two lanes and
+ * joins them again inside the call, so stream order as seen by the caller is unchanged.  The series are
+ * bit-identical to mode 0; sigma differs in its summation order only.  Measured on B200:
+ * slower than mode 0 for configs[2] (10.2 vs 9.9 ms per block) because the beamformer needs ~40 SMs' worth of
+ * issue slots to reach its HBM rate -- kept as an option, off by default. */
+LOFAR_API lofar_status lofar_plan_set_overlap(lofar_plan *plan, int mode, int chunk_slices);
 /* How lofar_run_block would cut a block of `slices`: slices per scratch chunk, and the number and
  * length (slices) of the independent time spans one inverse-PPF launch is divided into.  Host only;
  * lets tests aim parity windows at chunk and span boundaries. */
 LOFAR_API lofar_status lofar_plan_chunking(lofar_plan *plan, int slices, int64_t *chunk_slices,
                                            int *spans, int *span_slices);
+/* The same for chunk number `chunk` (0, 1, ...) of a block of `slices`: its first slice, its length
+ * (0 once `chunk` is past the end of the block; the last chunk may be shorter and is then cut into its own
+ * spans) and the spans of its inverse-PPF launch.  Host only. */
+LOFAR_API lofar_status lofar_plan_chunk_info(lofar_plan *plan, int slices, int chunk, int64_t *first_slice,
+                                             int64_t *chunk_slices, int *spans, int *span_slices);
 
 /* ---- stage calls (all pointers device) ------------------------------------------------------
  * X: [S][2][K][slices][re,im] int8 or int16, little endian, time fastest; base and row pitch

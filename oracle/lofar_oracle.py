@@ -29,14 +29,22 @@ CI8, CI16 = 0, 1
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (portable -O2, OpenMP; never tuned)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + f".tmp{os.getpid()}"
+    """Compile the oracle with gcc (portable -O2, OpenMP; never tuned).
+
+    LOFAR_ORACLE_SANITIZE=1 builds and loads an AddressSanitizer + UBSan copy instead (run the pins as
+    `LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 LOFAR_ORACLE_SANITIZE=1 python -m pytest
+    tests/test_oracle_pins.py tests/test_oracle_next_pins.py`)."""
+    san = os.environ.get("LOFAR_ORACLE_SANITIZE") == "1"
+    out = _LIB.replace(".so", "_san.so") if san else _LIB
+    flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] \
+        if san else ["-O2"]
+    if force or not os.path.exists(out) or os.path.getmtime(out) < os.path.getmtime(_SRC):
+        tmp = out + f".tmp{os.getpid()}"
         subprocess.check_call(
-            ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-fvisibility=hidden",
+            ["gcc", *flags, "-std=c11", "-fopenmp", "-fPIC", "-shared", "-fvisibility=hidden",
              "-o", tmp, _SRC, "-lm"])
-        os.replace(tmp, _LIB)
-    return _LIB
+        os.replace(tmp, out)
+    return out
 
 
 _lib = None

@@ -37,7 +37,8 @@ EXPORTS = (
     "lofar_plan_set_trigger", "lofar_plan_set_sigma_mode", "lofar_plan_set_inversion", "lofar_plan_set_dedispersion",
     "lofar_cluster", "lofar_requantize",
     "lofar_plan_workspace_bytes", "lofar_plan_set_allocator",
-    "lofar_plan_set_scratch_limit", "lofar_plan_chunking", "lofar_stream_state_bytes",
+    "lofar_plan_set_scratch_limit", "lofar_plan_set_overlap", "lofar_plan_chunking", "lofar_plan_chunk_info",
+    "lofar_stream_state_bytes",
     "lofar_stream_get_state", "lofar_stream_set_state", "lofar_beamform_dedisperse",
     "lofar_inverse_ppf", "lofar_trigger", "lofar_run_block", "lofar_stream_reset",
     "lofar_stream_push", "lofar_stream_sync", "lofar_plan_profile", "lofar_plan_profile_read",
@@ -83,7 +84,9 @@ def load() -> ctypes.CDLL:
         "lofar_plan_workspace_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
         "lofar_plan_set_allocator": (i, [vp, vp, vp, vp]),
         "lofar_plan_set_scratch_limit": (i, [vp, c.c_size_t]),
+        "lofar_plan_set_overlap": (i, [vp, i, i]),
         "lofar_plan_chunking": (i, [vp, i, c.POINTER(c.c_int64), c.POINTER(i), c.POINTER(i)]),
+        "lofar_plan_chunk_info": (i, [vp, i, i, c.POINTER(c.c_int64), c.POINTER(c.c_int64), c.POINTER(i), c.POINTER(i)]),
         "lofar_stream_state_bytes": (i, [vp, c.POINTER(c.c_size_t)]),
         "lofar_stream_get_state": (i, [vp, vp, c.c_size_t]),
         "lofar_stream_set_state": (i, [vp, vp, c.c_size_t]),
@@ -241,12 +244,26 @@ class Plan:
     def set_scratch_limit(self, nbytes: int):
         _check(self._lib.lofar_plan_set_scratch_limit(self._h, int(nbytes)), "lofar_plan_set_scratch_limit")
 
+    def set_overlap(self, mode: int, chunk_slices: int = 0):
+        _check(self._lib.lofar_plan_set_overlap(self._h, int(mode), int(chunk_slices)), "lofar_plan_set_overlap")
+
     def chunking(self, slices: int):
         """(slices per scratch chunk, spans per inverse-PPF launch, slices per span)."""
         zc, ns, sl = ctypes.c_int64(), ctypes.c_int(), ctypes.c_int()
         _check(self._lib.lofar_plan_chunking(self._h, slices, ctypes.byref(zc), ctypes.byref(ns), ctypes.byref(sl)),
                "lofar_plan_chunking")
         return int(zc.value), int(ns.value), int(sl.value)
+
+    def chunks(self, slices: int):
+        """[(first slice, slices, spans, slices per span)] for every scratch chunk of a block of `slices`."""
+        out = []
+        while True:
+            c0, nc, ns, sl = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int(), ctypes.c_int()
+            _check(self._lib.lofar_plan_chunk_info(self._h, slices, len(out), ctypes.byref(c0), ctypes.byref(nc),
+                                                   ctypes.byref(ns), ctypes.byref(sl)), "lofar_plan_chunk_info")
+            if nc.value == 0:
+                return out
+            out.append((int(c0.value), int(nc.value), int(ns.value), int(sl.value)))
 
     def get_state(self) -> np.ndarray:
         n = ctypes.c_size_t()

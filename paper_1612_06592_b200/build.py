@@ -5,7 +5,8 @@ nvcc cross-compiles without a GPU; the .so sits next to this file so that it tra
 
 Ablation builds (the measurements DESIGN.md section 8 quotes): `--define NAME [--define NAME ...] --out PATH` compiles a
 variant with -DNAME into PATH (objects under build/<names>/); run it with LOFAR_MOON_LIB=PATH, which the binding
-honours. Switches: LOFAR_FIR_SCALAR (synthesis FIR with scalar FFMA instead of packed FFMA2), LOFAR_ABLATE_STORES
+honours. Switches: LOFAR_FIR_SCALAR (synthesis FIR with scalar FFMA instead of packed FFMA2), LOFAR_FFT_SCALAR (the
+transform's complex adds / butterflies as scalar pairs instead of FADD2 / FFMA2), LOFAR_ABLATE_STORES
 (inverse PPF without its series stores), LOFAR_ABLATE_FIR (no FIR arithmetic), LOFAR_ABLATE_FFT (no transform
 arithmetic). Ablated variants compute wrong results by design; they exist to attribute time.
 """

@@ -66,6 +66,17 @@ void quiesce(lofar_plan *p)
 {
     if (p->s_copy) cudaStreamSynchronize(p->s_copy);
     if (p->s_comp) cudaStreamSynchronize(p->s_comp);
+    if (p->s_bf) cudaStreamSynchronize(p->s_bf);
+    if (p->s_ippf) cudaStreamSynchronize(p->s_ippf);
+}
+
+// SMs the inverse-PPF spans are planned for: with the two-lane pipeline a few SMs are left to the beamformer
+// (an inverse-PPF CTA owns the whole register file and shared memory of its SM, so nothing co-resides with it).
+int ippf_sm_budget(int num_sms, bool overlap)
+{
+    if (!overlap) return num_sms;
+    const int keep = num_sms - 16;
+    return keep > num_sms / 2 ? keep : num_sms / 2;
 }
 
 void free_tables(lofar_plan *p)
@@ -146,6 +157,7 @@ struct Layout {
     long long xhat_pitch;
     size_t x_bytes, cand, sigma;   // streaming staging (per slot)
     long long cap, zchunk, nsteps;
+    bool overlap;            // two-lane pipeline: two scratch slots of zchunk slices each
     size_t table_bytes() const
     {
         return (W + Dph + gs + tw + Z) * sizeof(float2) + wimg * sizeof(unsigned short) +
@@ -173,8 +185,18 @@ Layout layout(const lofar_plan *p)
     long long zc = (long long)(p->scratch_limit / (B * K * sizeof(float2)));
     zc = zc >= 1024 ? zc / 1024 * 1024 : zc / 32 * 32;
     if (zc < 32) zc = 32;
+    // Two-lane pipeline: only with the tensor-core beamformer (a few SMs keep it at its HBM rate) and only if the
+    // block then has at least two chunks; the two slots share the scratch budget.
+    L.overlap = p->overlap != 0 && L.tc && p->B >= p->tc_min_beams;
+    if (L.overlap) {
+        long long zo = zc / 2;
+        if (zo > p->overlap_chunk) zo = p->overlap_chunk;
+        zo = zo >= 1024 ? zo / 1024 * 1024 : zo / 32 * 32;
+        if (zo < 32 || L.cap <= zo) L.overlap = false;     // a single chunk: nothing to pipeline
+        else zc = zo;
+    }
     L.zchunk = round_up(zc < L.cap ? zc : L.cap, 32);      // whole 32-slice tiles of the scratch layout
-    L.Z = B * K * (size_t)L.zchunk;
+    L.Z = B * K * (size_t)L.zchunk * (L.overlap ? 2 : 1);
     L.nsteps = L.cap / kStepSlices;
     L.partial = ns * (size_t)L.nsteps;
     L.chunkmax = ns * (size_t)L.nsteps;
@@ -284,6 +306,21 @@ lofar_status build(lofar_plan *p)
 
     // ---- scratch sized for max_slices ----
     p->zchunk = L.zchunk;
+    p->overlap_on = L.overlap;
+    p->ippf_sms = ippf_sm_budget(p->num_sms, L.overlap);
+    if (L.overlap && !p->s_bf) {
+        // the inverse PPF goes first wherever both kernels have CTAs pending; the beamformer fills what is left
+        int least = 0, greatest = 0;
+        CU(cudaDeviceGetStreamPriorityRange(&least, &greatest));
+        CU(cudaStreamCreateWithPriority(&p->s_ippf, cudaStreamNonBlocking, greatest));
+        CU(cudaStreamCreateWithPriority(&p->s_bf, cudaStreamNonBlocking, least));
+        CU(cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming));
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaEventCreateWithFlags(&p->ev_bf[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&p->ev_ippf[i], cudaEventDisableTiming));
+        }
+    }
     if ((st = dev_alloc(p, &p->dZ, L.Z)) != LOFAR_OK) return st;
     CU(cudaMemset(p->dZ, 0, L.Z * sizeof(float2)));
     p->partial_pitch = (int)L.nsteps;
@@ -362,11 +399,13 @@ lofar_status ensure(lofar_plan *p, int slices)
     return LOFAR_OK;
 }
 
-// Spans of the inverse-PPF launch: minimise (waves of CTAs) x (steps per span + warm-up step).
-void plan_spans(long long nsteps, int nseries, int sms, int *nspans, int *span_len)
+// Spans of the inverse-PPF launch: minimise (waves of CTAs) x (steps per span + warm-up step). one_wave: at most
+// `sms` CTAs (the two-lane pipeline leaves the other SMs to the beamformer for the whole launch).
+void plan_spans(long long nsteps, int nseries, int sms, bool one_wave, int *nspans, int *span_len)
 {
     long long best_cost = -1, best = 1;
-    const long long lim = nsteps < 4096 ? nsteps : 4096;
+    long long lim = nsteps < 4096 ? nsteps : 4096;
+    if (one_wave && nseries <= sms && lim > sms / nseries) lim = sms / nseries;
     for (long long n = 1; n <= lim; ++n) {
         const long long per = (nsteps + n - 1) / n;
         const long long real = (nsteps + per - 1) / per;
@@ -404,6 +443,9 @@ lofar_status lsmr_solve(lofar_plan *p, long long T, float *series, long long ser
     return LOFAR_OK;
 }
 
+// True while a block call runs its chunks through the two-lane pipeline (set by run_block_impl).
+bool lanes_now(const lofar_plan *p, long long) { return p->lanes_active; }
+
 struct EmitTo { lofar_candidate *cand; uint32_t *count; };   // cand == nullptr: no emission from the epilogue
 
 lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, int ztile, long long nc, int zmap_trials,
@@ -421,7 +463,9 @@ lofar_status do_ippf(lofar_plan *p, const float2 *Z, long long zpitch, int ztile
     a.series = series; a.series_pitch = series_pitch; a.out0 = out0;
     a.Dph = p->dDph; a.zmap_trials = zmap_trials;
     a.K = p->K; a.k0 = p->k0; a.nseries = p->ninv();
-    plan_spans((nc + kStepSlices - 1) / kStepSlices, a.nseries, p->num_sms, &a.nspans, &a.span_len);
+    const bool lanes = ztile && lanes_now(p, nc);
+    plan_spans((nc + kStepSlices - 1) / kStepSlices, a.nseries, lanes ? p->ippf_sms : p->num_sms, lanes, &a.nspans,
+               &a.span_len);
     a.hist_in = p->dHist[p->hist_parity];
     a.hist_out = p->dHist[p->hist_parity ^ 1];
     a.gs = p->dGs; a.tw = p->dTw;
@@ -489,23 +533,48 @@ lofar_status run_block_impl(lofar_plan *p, const void *X, int slices, float *ser
         CU(cudaMemcpyAsync(p->dHist0, p->dHist[p->hist_parity], (size_t)ns * (kTaps - 1) * kMfft * sizeof(float),
                            cudaMemcpyDeviceToDevice, st));
     int partial0 = 0;
-    for (long long c0 = 0; c0 < T; c0 += p->zchunk) {
+    // Chunk loop. Serial: both kernels of every chunk on the caller's stream. Two-lane pipeline (overlap_on): the
+    // beamformer of chunk c + 1 runs on s_bf while the inverse PPF of chunk c runs on s_ippf; the two alternate
+    // between the two scratch slots, chained by events; the caller's stream forks before and joins after the loop.
+    const bool lanes = p->overlap_on && T > p->zchunk;
+    p->lanes_active = lanes;
+    cudaStream_t sb = lanes ? p->s_bf : st, si = lanes ? p->s_ippf : st;
+    if (lanes) {
+        CU(cudaEventRecord(p->ev_fork, st));
+        CU(cudaStreamWaitEvent(sb, p->ev_fork, 0));
+        CU(cudaStreamWaitEvent(si, p->ev_fork, 0));
+    }
+    const size_t zslot = (size_t)p->B * p->K * (size_t)p->zchunk;
+    int ci = 0;
+    for (long long c0 = 0; c0 < T; c0 += p->zchunk, ++ci) {
         const long long nc = (T - c0 < p->zchunk) ? T - c0 : p->zchunk;
+        const int slot = lanes ? (ci & 1) : 0;
+        float2 *Zc = p->dZ + (size_t)slot * zslot;
         BeamformArgs b{};
         b.X = X; b.xpitch = T; b.t0 = c0; b.nt = nc;
-        b.Z = p->dZ; b.zpitch = p->zchunk; b.ztile = 1;
+        b.Z = Zc; b.zpitch = p->zchunk; b.ztile = 1;
         b.W = p->dW; b.Dph = p->dDph;
         b.S = p->S; b.K = p->K; b.B = p->B; b.nphase = 0; b.dtype = p->dtype;
+        if (lanes && ci >= 2) CU(cudaStreamWaitEvent(sb, p->ev_ippf[slot], 0));   // the slot has been consumed
         {
-            ProfScope prof(p, 0, st);
-            const int n = beamform_dispatch(p, b, st);
+            ProfScope prof(p, 0, sb);
+            const int n = beamform_dispatch(p, b, sb);
             if (n < 0) return LOFAR_E_CUDA;
             p->launches += n;
         }
-        lofar_status s = do_ippf(p, p->dZ, p->zchunk, 1, nc, ztrials, lsmr ? nullptr : inv_series, inv_pitch, c0 * kMfft,
-                                 &partial0, c0 / kStepSlices, st, emit ? EmitTo{cand, count} : EmitTo{nullptr, nullptr},
+        if (lanes) {
+            CU(cudaEventRecord(p->ev_bf[slot], sb));
+            CU(cudaStreamWaitEvent(si, p->ev_bf[slot], 0));
+        }
+        lofar_status s = do_ippf(p, Zc, p->zchunk, 1, nc, ztrials, lsmr ? nullptr : inv_series, inv_pitch, c0 * kMfft,
+                                 &partial0, c0 / kStepSlices, si, emit ? EmitTo{cand, count} : EmitTo{nullptr, nullptr},
                                  lsmr);
         if (s != LOFAR_OK) return s;
+        if (lanes) CU(cudaEventRecord(p->ev_ippf[slot], si));
+    }
+    if (lanes) {
+        CU(cudaEventRecord(p->ev_join, si));                 // every beamformer launch has been waited for by s_ippf
+        CU(cudaStreamWaitEvent(st, p->ev_join, 0));
     }
     if (lsmr) { const lofar_status s1 = lsmr_solve(p, T, inv_series, inv_pitch, st); if (s1 != LOFAR_OK) return s1; }
     if (exact) {
@@ -602,9 +671,15 @@ void lofar_plan_destroy(lofar_plan *p)
     free_tables(p);                    // drains the plan's own streams first
     if (p->s_copy) { cudaStreamDestroy(p->s_copy); p->s_copy = nullptr; }
     if (p->s_comp) { cudaStreamDestroy(p->s_comp); p->s_comp = nullptr; }
+    if (p->s_bf) { cudaStreamDestroy(p->s_bf); p->s_bf = nullptr; }
+    if (p->s_ippf) { cudaStreamDestroy(p->s_ippf); p->s_ippf = nullptr; }
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     for (int i = 0; i < 2; ++i) {
         if (p->ev_copied[i]) cudaEventDestroy(p->ev_copied[i]);
         if (p->ev_done[i]) cudaEventDestroy(p->ev_done[i]);
+        if (p->ev_bf[i]) cudaEventDestroy(p->ev_bf[i]);
+        if (p->ev_ippf[i]) cudaEventDestroy(p->ev_ippf[i]);
     }
     if (p->hCount) cudaFreeHost(p->hCount);
     for (auto &r : p->prof_pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
@@ -730,24 +805,44 @@ lofar_status lofar_plan_set_scratch_limit(lofar_plan *p, size_t bytes)
     return LOFAR_OK;
 }
 
-lofar_status lofar_plan_chunking(lofar_plan *p, int slices, int64_t *chunk_slices, int *spans, int *span_slices)
+lofar_status lofar_plan_set_overlap(lofar_plan *p, int mode, int chunk_slices)
 {
-    if (!p || slices <= 0 || !chunk_slices || !spans || !span_slices) return LOFAR_E_INVALID;
+    if (!p || (mode != 0 && mode != 1) || chunk_slices < 0) return LOFAR_E_INVALID;
+    p->overlap = mode;
+    p->overlap_chunk = chunk_slices > 0 ? chunk_slices : 8192;
+    p->built = false;
+    return LOFAR_OK;
+}
+
+lofar_status lofar_plan_chunk_info(lofar_plan *p, int slices, int chunk, int64_t *first_slice, int64_t *chunk_slices,
+                                   int *spans, int *span_slices)
+{
+    if (!p || slices <= 0 || chunk < 0 || !first_slice || !chunk_slices || !spans || !span_slices) return LOFAR_E_INVALID;
     if (p->max_slices > 0 && slices > p->max_slices) return LOFAR_E_STATE;
     const int keep = p->max_slices;
     if (p->max_slices <= 0) p->max_slices = slices;
     const Layout L = layout(p);
     p->max_slices = keep;
-    *chunk_slices = L.zchunk;
     int sms = p->num_sms;
     if (!p->built) {
         int dev = 0;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         else { cudaGetLastError(); sms = 148; }
     }
-    const long long nc = slices < L.zchunk ? slices : L.zchunk;
-    plan_spans((nc + kStepSlices - 1) / kStepSlices, p->B * p->D, sms, spans, span_slices);
+    const long long c0 = (long long)chunk * L.zchunk;
+    *first_slice = c0; *chunk_slices = 0; *spans = 0; *span_slices = 0;
+    if (c0 >= slices) return LOFAR_OK;                       // past the last chunk
+    const long long nc = slices - c0 < L.zchunk ? slices - c0 : L.zchunk;
+    const bool lanes = L.overlap && slices > L.zchunk;
+    *chunk_slices = nc;
+    plan_spans((nc + kStepSlices - 1) / kStepSlices, p->ninv(), ippf_sm_budget(sms, lanes), lanes, spans, span_slices);
     return LOFAR_OK;
+}
+
+lofar_status lofar_plan_chunking(lofar_plan *p, int slices, int64_t *chunk_slices, int *spans, int *span_slices)
+{
+    int64_t first = 0;
+    return lofar_plan_chunk_info(p, slices, 0, &first, chunk_slices, spans, span_slices);
 }
 
 lofar_status lofar_beamform_dedisperse(lofar_plan *p, const void *X, int slices, void *Z, void *stream)

@@ -12,9 +12,19 @@ typedef unsigned long long u64;
 __device__ __forceinline__ u64 PK(float x, float y) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y)); return r; }
 __device__ __forceinline__ float LO(u64 v) { float x; asm("{\n\t.reg .f32 t;\n\tmov.b64 {%0, t}, %1;\n\t}" : "=f"(x) : "l"(v)); return x; }
 __device__ __forceinline__ float HI(u64 v) { float y; asm("{\n\t.reg .f32 t;\n\tmov.b64 {t, %0}, %1;\n\t}" : "=f"(y) : "l"(v)); return y; }
+// fma2p is always the packed instruction (the synthesis FIR); add2 / sub2 / fma2 are the transform's arithmetic and
+// become scalar pairs with -DLOFAR_FFT_SCALAR (ablation: packed instructions with distinct register operands are
+// register-file limited to ~79 FMA/clk/SM against ~100 for scalar ones, but take half the issue slots).
+__device__ __forceinline__ u64 fma2p(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+#ifdef LOFAR_FFT_SCALAR
+__device__ __forceinline__ u64 add2(u64 a, u64 b) { return PK(LO(a) + LO(b), HI(a) + HI(b)); }
+__device__ __forceinline__ u64 sub2(u64 a, u64 b) { return PK(LO(a) - LO(b), HI(a) - HI(b)); }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { return PK(fmaf(LO(a), LO(b), LO(c)), fmaf(HI(a), HI(b), HI(c))); }
+#else
 __device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 d; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { return fma2p(a, b, c); }
+#endif
 __device__ __forceinline__ u64 lds64(const float2 *p) { return *reinterpret_cast<const u64 *>(p); }
 __device__ __forceinline__ void sts64(float2 *p, u64 v) { *reinterpret_cast<u64 *>(p) = v; }
 // a * (c + i s), scalar products (a complex product needs the swapped pair, which the packed forms lack)

@@ -219,7 +219,7 @@ __device__ __forceinline__ u64 fir_fma(u64 g, u64 x, u64 acc)
 #ifdef LOFAR_FIR_SCALAR
     return PK(fmaf(LO(g), LO(x), LO(acc)), fmaf(HI(g), HI(x), HI(acc)));
 #else
-    return fma2(g, x, acc);
+    return fma2p(g, x, acc);
 #endif
 }
 
@@ -249,7 +249,7 @@ __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, 
 #ifndef LOFAR_ABLATE_STORES
                 if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)j * kM + 2 * tid), make_float2(vx, vy));
 #endif
-                ssum2 = fma2(acc[j], acc[j], ssum2);
+                ssum2 = fma2p(acc[j], acc[j], ssum2);
                 smax = fmaxf(smax, fmaxf(fabsf(vx), fabsf(vy)));
             }
         }

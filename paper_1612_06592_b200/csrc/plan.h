@@ -167,7 +167,16 @@ struct lofar_plan {
     void *(*alloc_fn)(size_t, void *) = nullptr;
     void (*free_fn)(void *, void *) = nullptr;
     void *alloc_ctx = nullptr;
-    size_t scratch_limit = (size_t)4 << 30;   // bytes of beam-sum scratch per time chunk
+    size_t scratch_limit = (size_t)4 << 30;   // bytes of beam-sum scratch (all slots together)
+    // Two-lane block pipeline (lofar_plan_set_overlap): the beamformer of chunk c+1 runs on a low-priority stream
+    // beside the inverse PPF of chunk c, on the SMs the inverse PPF leaves free; two scratch slots.
+    int overlap = 0;                   // requested: 0 = serial (default: measured faster), 1 = pipeline
+    long long overlap_chunk = 8192;    // slices per chunk of the pipeline (fill + drain = one chunk of each kernel)
+    bool lanes_active = false;         // the block call in progress uses the pipeline (more than one chunk)
+    bool overlap_on = false;           // decided by build(): tensor-core beamformer and at least two chunks
+    int ippf_sms = 148;                // SMs the inverse-PPF spans are planned for (num_sms minus the reserve)
+    cudaStream_t s_bf = nullptr, s_ippf = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_bf[2] = {nullptr, nullptr}, ev_ippf[2] = {nullptr, nullptr};
     // device state
     bool built = false;
     bool reset_pending = false;        // carried state is zeroed on the stream of the next compute call

@@ -136,6 +136,37 @@ def test_scratch_chunks_hand_over_history(torch, oracle, T, limit_slices):
     p.destroy()
 
 
+@pytest.mark.parametrize("T,chunk", [(200, 64), (264, 32)])
+def test_two_lane_pipeline_matches_oracle(torch, oracle, T, chunk):
+    """lofar_plan_set_overlap(1): the beamformer of chunk c + 1 on one plan stream beside the inverse PPF of chunk c
+    on another, alternating scratch slots, fork / join with the caller's stream. Same results as the oracle, and
+    bit-identical series to the serial mode; two blocks, so that the slot and history hand-over across the join is
+    covered as well."""
+    w, tau, X = _case(S=4, B=5, K=24, k0=200, T=T, dtype="ci8", kappa=4.0, n_pulses=2)
+    pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa)
+    ref, sig_ref, _, _ = pipe.run_block(X)
+    X1 = synth.generate_block(w, 1, tau=tau)
+    ref1, sig1, _, _ = pipe.run_block(X1)
+    p = binding.plan_for(w, tau)
+    p.set_overlap(1, chunk)
+    chunks = p.chunks(T)
+    assert len(chunks) == -(-T // chunk) and all(c[1] <= chunk for c in chunks) and sum(c[1] for c in chunks) == T
+    q = binding.plan_for(w, tau)                     # serial twin
+    q.set_scratch_limit(w.B * w.K * 8 * chunk)
+    for blk, (Xb, rb, sb) in enumerate(((X, ref, sig_ref), (X1, ref1, sig1))):
+        got, rec, n, sigma = _run(torch, p, Xb, T)
+        ser, _, _, sig_serial = _run(torch, q, Xb, T)
+        assert np.array_equal(got, ser)
+        np.testing.assert_allclose(sigma, sig_serial, rtol=1e-6)
+        for s in range(w.nseries):
+            assert_close(got[s], rb[s], f"series {s}")
+        np.testing.assert_allclose(sigma, sb, rtol=5e-6)
+        env, sig = oracle_snr(oracle, rb, 1)
+        check_candidates(rec, n, env, sig, w.B, w.D, w.kappa, offset=blk * T * 1024)
+    p.destroy()
+    q.destroy()
+
+
 def test_int8_minimum_on_the_tensor_core_path(torch, oracle):
     """-128 is legal int8 input; the tcgen05 kernel (B >= 4) converts bytes to fp16 through an
     offset trick that must stay exact at the end of the range, also for -128 + -128 = -256."""

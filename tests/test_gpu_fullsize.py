@@ -88,12 +88,12 @@ def _boundaries(plan, T):
     each launch (first, second, middle, last), the last tile."""
     zc, nspans, span = plan.chunking(T)
     out = set()
-    for c0 in range(0, T, zc):
-        nc = min(zc, T - c0)
-        _, ns, sl = plan.chunking(nc) if nc != zc else (zc, nspans, span)
+    chunks = plan.chunks(T)
+    aimed = {0, 1, len(chunks) // 2, len(chunks) - 1}        # span starts: first, second, middle and last (ragged) chunk
+    for i, (c0, nc, ns, sl) in enumerate(chunks):
         if c0:
-            out.add(c0)
-        for j in sorted({1, 2, ns // 2, ns - 1}):
+            out.add(c0)                                      # every chunk hand-over (both scratch slots of the pipeline)
+        for j in sorted({1, 2, ns // 2, ns - 1}) if i in aimed else [1 + i % max(1, ns - 1)]:
             if 0 < j < ns and j * sl < nc:
                 out.add(c0 + j * sl)
     out.add(T - 16)
