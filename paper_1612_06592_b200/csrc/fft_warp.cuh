@@ -12,7 +12,7 @@ typedef unsigned long long u64;
 __device__ __forceinline__ u64 PK(float x, float y) { u64 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y)); return r; }
 __device__ __forceinline__ float LO(u64 v) { float x; asm("{\n\t.reg .f32 t;\n\tmov.b64 {%0, t}, %1;\n\t}" : "=f"(x) : "l"(v)); return x; }
 __device__ __forceinline__ float HI(u64 v) { float y; asm("{\n\t.reg .f32 t;\n\tmov.b64 {t, %0}, %1;\n\t}" : "=f"(y) : "l"(v)); return y; }
-// fma2p is always the packed instruction (the synthesis FIR); add2 / sub2 / fma2 are the transform's arithmetic and
+// fma2p is always the packed instruction; add2 / sub2 / fma2 are the transform's arithmetic and
 // become scalar pairs with -DLOFAR_FFT_SCALAR (ablation: packed instructions with distinct register operands are
 // register-file limited to ~79 FMA/clk/SM against ~100 for scalar ones, but take half the issue slots).
 __device__ __forceinline__ u64 fma2p(u64 a, u64 b, u64 c) { u64 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
@@ -84,16 +84,23 @@ template <bool TW>
 __device__ __forceinline__ void fft512_pass_b(float2 *row, const float2 *stw, int lane)
 {
     u64 x[16];
+    // pad(lane + 32 r) = lane + (lane >> 4) + 34 r: one base pointer and compile-time offsets (the compiler does not
+    // fold the shift inside pad() by itself and would spend three integer instructions per access)
+    const float2 *src = row + lane + (lane >> 4);
     if (TW) {
         const float2 *T = stw + 256 + lane;      // T[32 r' + lane] = exp(2 pi i j (hh + 2 r') / 512)
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
             const float2 t = T[32 * r];
-            x[r] = cmulp(lds64(row + pad(lane + 32 * r)), t.x, t.y);
+            x[r] = cmulp(lds64(src + 34 * r), t.x, t.y);
         }
     } else {
 #pragma unroll
+#ifdef LOFAR_PB_OLDLD
         for (int r = 0; r < 16; ++r) x[r] = lds64(row + pad(lane + 32 * r));
+#else
+        for (int r = 0; r < 16; ++r) x[r] = lds64(src + 34 * r);
+#endif
     }
     idft16p(x);
     const bool hi = lane >= 16;
@@ -120,9 +127,14 @@ __device__ __forceinline__ void fft512_pass_b(float2 *row, const float2 *stw, in
         x[m] = fma2(x[m], sg, other);
     }
     __syncwarp();
-    const int base = (lane & 15) + (hi ? 256 : 0);
+    // pad(base + 16 m) = base + (base >> 4) + 17 m with base = (lane & 15) + (hi ? 256 : 0)
+    float2 *dst = row + (lane & 15) + (hi ? 256 + 16 : 0);
 #pragma unroll
-    for (int m = 0; m < 16; ++m) sts64(row + pad(base + 16 * m), x[m]);
+#ifdef LOFAR_PB_OLDST
+    for (int m = 0; m < 16; ++m) sts64(row + pad((lane & 15) + (hi ? 256 : 0) + 16 * m), x[m]);
+#else
+    for (int m = 0; m < 16; ++m) sts64(dst + 17 * m, x[m]);
+#endif
     __syncwarp();
 }
 
@@ -132,12 +144,14 @@ __device__ __forceinline__ void fft512_pass_b(float2 *row, const float2 *stw, in
 __device__ __forceinline__ void fft512_warp(float2 *row, const float2 *stw, int lane)
 {
     u64 x[16];
+    const float2 *src = row + lane + (lane >> 4);          // pad(lane + 32 r) = lane + (lane >> 4) + 34 r
 #pragma unroll
-    for (int r = 0; r < 16; ++r) x[r] = lds64(row + pad(lane + 32 * r));
+    for (int r = 0; r < 16; ++r) x[r] = lds64(src + 34 * r);
     idft16p(x);
     __syncwarp();
+    float2 *dst = row + 17 * lane;                         // pad(16 lane + m) = 17 lane + m
 #pragma unroll
-    for (int m = 0; m < 16; ++m) sts64(row + pad(16 * lane + m), x[m]);
+    for (int m = 0; m < 16; ++m) sts64(dst + m, x[m]);
     __syncwarp();
     fft512_pass_b<true>(row, stw, lane);
 }

@@ -15,8 +15,11 @@
 //   FIR      : thread n owns output residues r = 2n, 2n+1 and keeps their 16 tap pairs in registers; the
 //              31-slice window (15 carried + 16 new) is read from the previous and current slice buffers;
 //              16 x 1024 contiguous output samples are written per step.
-// Complex adds and the FIR run on the packed fp32x2 instructions (FADD2 / FFMA2): the same FMA-pipe
-// throughput as the scalar forms for half the issue slots (the kernel is issue-bound).
+// The transform's complex adds and butterflies are packed fp32x2 instructions (FADD2 / FFMA2: half the issue slots in
+// phases that are issue-bound); the FIR is scalar FFMA (the packed form with three distinct register operands is
+// register-file limited). Launch parameters are read from the constant bank where they are used and slice indices
+// are 32-bit, which keeps the persistent register state small: the kernel sits at the 128-register cap and every
+// register the scheduler gets back shows in the FIR.
 // The 15-slice history lives in the "previous" buffer, is loaded from the plan at the start of a block and
 // written back by the CTA that owns the last span; CTAs that start in the middle of a block first
 // transform the 16 slices before their span (no output).
@@ -28,8 +31,8 @@ namespace {
 
 constexpr int kThreads = 512;
 constexpr int kTwCount = 256 + 512;        // w1024[256], TB[32][16] = exp(2 pi i j r / 512)
-constexpr int kStageF2 = kH * kStep;       // stage: up to 512 rows x 16 slices of float2 = 64 KB
-constexpr size_t kSmemBytes = (size_t)(2 * kStep * kRow + kStageF2 + kTwCount + kH) * sizeof(float2) + 256;
+constexpr int kStageF2 = (kH + 1) * kStep; // stage: bins 0..512 x 16 slices of float2 (row 512 stays zero)
+constexpr size_t kSmemBytes = (size_t)(2 * kStep * kRow + kStageF2 + kTwCount + kH + 1) * sizeof(float2) + 256;
 
 // ---- mbarrier + bulk asynchronous copy (TMA unit, SASS UBLKCP / SYNCS) ------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -54,40 +57,34 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
                  :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
-struct Ctx {
-    const float2 *Zs;      // this series' beam sums
-    const float2 *ph;      // trial phasors of this series or nullptr
-    long long zpitch, nc;
-    int K, k0, bulk_rows, tiled;
-};
-
 // Brings the K rows x 16 slices of the step starting at slice q into rows k0 .. k0 + K - 1 of the stage (`stage` points at row k0).
-// Returns true if the copy is asynchronous (completion on the mbarrier), false if the threads stored it.
-__device__ __forceinline__ bool stage_fill(const Ctx &c, long long q, float2 *stage, uint32_t bar, int tid)
+// Zs: this series' beam sums. Returns true if the copy is asynchronous (completion on the mbarrier), false if the
+// threads stored it. The launch parameters are read where they are used (constant bank), not kept in registers.
+__device__ __forceinline__ bool stage_fill(const IppfArgs &a, const float2 *Zs, int q, float2 *stage, uint32_t bar, int tid)
 {
-    if (c.tiled) {
+    if (a.ztile) {
         // plan scratch [tile = q/16][K][16]: the whole step is one contiguous block
         if (tid == 0) {
-            const uint32_t bytes = (uint32_t)c.K * 128u;
+            const uint32_t bytes = (uint32_t)a.K * 128u;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the stage was last read by ordinary loads
             mbar_arrive_expect_tx(bar, bytes);
-            bulk_g2s(smem_u32(stage), c.Zs + (size_t)(q >> 4) * c.K * 16, bytes, bar);
+            bulk_g2s(smem_u32(stage), Zs + (size_t)(q >> 4) * a.K * 16, bytes, bar);
         }
         return true;
     }
-    if (c.bulk_rows && q + kStep <= c.nc) {
+    if (a.vec_ok && q + kStep <= a.nc) {
         // caller's Z [K][zpitch]: one 128-byte line per row
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        if (tid == 0) mbar_arrive_expect_tx(bar, (uint32_t)c.K * 128u);
-        for (int j = tid; j < c.K; j += kThreads)
-            bulk_g2s(smem_u32(stage + j * kStep), c.Zs + (size_t)j * c.zpitch + q, 128u, bar);
+        if (tid == 0) mbar_arrive_expect_tx(bar, (uint32_t)a.K * 128u);
+        for (int j = tid; j < a.K; j += kThreads)
+            bulk_g2s(smem_u32(stage + j * kStep), Zs + (size_t)j * a.zpitch + q, 128u, bar);
         return true;
     }
     // ragged or unaligned: plain loads, zero beyond the end of the launch
-    for (int idx = tid; idx < c.K * kStep; idx += kThreads) {
+    for (int idx = tid; idx < a.K * kStep; idx += kThreads) {
         const int j = idx >> 4, t = idx & 15;
         float2 v = make_float2(0.f, 0.f);
-        if (q + t < c.nc) v = c.Zs[(size_t)j * c.zpitch + q + t];
+        if (q + t < a.nc) v = Zs[(size_t)j * a.zpitch + q + t];
         stage[idx] = v;
     }
     return false;
@@ -120,45 +117,42 @@ __device__ __forceinline__ void vpair(u64 a, u64 b, float2 w, u64 &vm, u64 &vmir
 }
 
 // All 512 threads, one step: thread (j, t) -- j = residue of the bin index mod 32, t = slice of the step -- builds
-// V[j + 32 r], r = 0..15, of its slice straight from the stage ([512][16], so the 16 slices of a half-warp read one
+// V[j + 32 r], r = 0..15, of its slice straight from the stage ([513][16], so the 16 slices of a half-warp read one
 // 128-byte line), does the 16-point DFT over r, applies the radix-32 twiddles exp(2 pi i j m / 512) and stores
 // the result slice-major at dst[t][pad(16 j + m)]. The mirror of bin j + 32 r is bin (32 - j) + 32 (15 - r): a
 // warp holds j in its low and 32 - j in its high half, each thread forms the pairs r = 0..7 and hands the
-// mirrored values to its partner lane (shuffle); warp 0 holds the two self-paired residues j = 0 and j = 16.
+// mirrored values to its partner lane (shuffle). Warp 0 holds the two self-paired residues j = 0 and j = 16: the same
+// code with the lane itself as partner; for j = 0 the pairs are (32 r, 32 (16 - r)), i.e. the mirrored values land one
+// place further (fixed up below), bin 0 keeps its real part only and pairs with the always-zero row 512 (reading A10),
+// and bin 256 is its own mirror. One code path for all warps keeps the loop body inside the instruction cache.
 template <bool PH>
 __device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, float2 *dst, const float2 *stw, int tid)
 {
     const int warp = tid >> 5, lane = tid & 31, half = lane >> 4, t = lane & 15;
     constexpr int R = 32 * kStep;                  // stage elements between bins m and m + 32
+    const int j = half ? (warp ? 32 - warp : 16) : warp;
+    const bool dc = (warp | half) == 0;            // the thread that holds bins 0, 32, ..., 480
     u64 x[16];
-    int j;
+    const float2 *sa = stage + j * kStep + t, *sb = stage + (512 - j) * kStep + t;
+    const float2 *pa = sph + j, *pb = sph + 512 - j, *wj = stw + j;
+    u64 give[8];
+    {
+        u64 a0 = ldz<PH>(sa, pa);
+        if (dc) a0 = PK(LO(a0), 0.f);
+        vpair(a0, ldz<PH>(sb, pb), wj[0], x[0], give[0]);
+    }
+#pragma unroll
+    for (int r = 1; r < 8; ++r) vpair(ldz<PH>(sa + r * R, pa + 32 * r), ldz<PH>(sb - r * R, pb - 32 * r), wj[32 * r], x[r], give[r]);
+    const int partner = warp ? lane ^ 16 : lane;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) x[15 - r] = __shfl_sync(0xffffffffu, give[r], partner);
     if (warp == 0) {
-        const float2 *s0 = stage + t;
-        if (half == 0) {
-            j = 0;
-            const u64 y0 = ldz<PH>(s0, sph), y256 = ldz<PH>(s0 + 256 * kStep, sph + 256);
-            x[0] = PK(LO(y0), LO(y0));                              // prepass_dc
+        const u64 y256 = ldz<PH>(stage + 256 * kStep + t, sph + 256);
+        if (dc) {
+#pragma unroll
+            for (int m = 15; m > 8; --m) x[m] = x[m - 1];           // mirror of bin 32 r is bin 32 (16 - r)
             x[8] = PK(2.0f * LO(y256), -2.0f * HI(y256));           // prepass_quarter
-#pragma unroll
-            for (int r = 1; r < 8; ++r)
-                vpair(ldz<PH>(s0 + r * R, sph + 32 * r), ldz<PH>(s0 + (16 - r) * R, sph + 512 - 32 * r), stw[32 * r], x[r],
-                      x[16 - r]);
-        } else {
-            j = 16;
-#pragma unroll
-            for (int r = 0; r < 8; ++r)
-                vpair(ldz<PH>(s0 + 16 * kStep + r * R, sph + 16 + 32 * r),
-                      ldz<PH>(s0 + 16 * kStep + (15 - r) * R, sph + 496 - 32 * r), stw[16 + 32 * r], x[r], x[15 - r]);
         }
-    } else {
-        j = half ? 32 - warp : warp;
-        const float2 *sa = stage + j * kStep + t, *sb = stage + (512 - j) * kStep + t;
-        const float2 *pa = sph + j, *pb = sph + 512 - j, *wj = stw + j;
-        u64 give[8];
-#pragma unroll
-        for (int r = 0; r < 8; ++r) vpair(ldz<PH>(sa + r * R, pa + 32 * r), ldz<PH>(sb - r * R, pb - 32 * r), wj[32 * r], x[r], give[r]);
-#pragma unroll
-        for (int r = 0; r < 8; ++r) x[15 - r] = __shfl_xor_sync(0xffffffffu, give[r], 16);
     }
     idft16p(x);
     const float2 *T = stw + 256 + 16 * j;          // T[m] = exp(2 pi i j m / 512)
@@ -170,16 +164,6 @@ __device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, f
         sts64(row + m, cmulp(x[m], f.x, f.y));
     }
 }
-
-// Where candidates found in the FIR epilogue go (threshold known before the block: causal sigma, or the rescan).
-struct Emit {
-    lofar_candidate *cand;
-    uint32_t *count;
-    uint32_t cap;
-    uint32_t series, trial;
-    float thr, sigma;        // thr = kappa * sigma; +inf disables emission
-    uint64_t sample0;        // global index of sample 0 of the series slice the step starts at
-};
 
 // Rare path, kept out of line and out of the FIR's registers: a thread whose step maximum exceeds the threshold
 // recomputes its 2 x 16 outputs (taps re-read from global memory) and records every sample above the threshold
@@ -213,13 +197,15 @@ __device__ __noinline__ void emit_step(const float2 *prev, const float2 *cur, co
     }
 }
 
-// One tap of the FIR on a residue pair: packed FFMA2 (half the issue slots) or, with -DLOFAR_FIR_SCALAR, two FFMA.
+// One tap of the FIR on a residue pair: two scalar FFMA. The packed FFMA2 (-DLOFAR_FIR_PACKED) takes half the issue
+// slots but, with three distinct register operands, is register-file limited to ~79 FMA/clk/SM against ~100 for the
+// scalar form (micro-benchmark); measured in the kernel: 6.05 ms scalar, 6.29 ms packed.
 __device__ __forceinline__ u64 fir_fma(u64 g, u64 x, u64 acc)
 {
-#ifdef LOFAR_FIR_SCALAR
-    return PK(fmaf(LO(g), LO(x), LO(acc)), fmaf(HI(g), HI(x), HI(acc)));
-#else
+#ifdef LOFAR_FIR_PACKED
     return fma2p(g, x, acc);
+#else
+    return PK(fmaf(LO(g), LO(x), LO(acc)), fmaf(HI(g), HI(x), HI(acc)));
 #endif
 }
 
@@ -247,7 +233,11 @@ __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, 
             if (FULL || j < nvalid) {
                 const float vx = LO(acc[j]), vy = HI(acc[j]);
 #ifndef LOFAR_ABLATE_STORES
-                if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)j * kM + 2 * tid), make_float2(vx, vy));
+#ifdef LOFAR_ST_PLAIN
+                if (out) *reinterpret_cast<float2 *>(out + (size_t)j * kM + 2 * tid) = make_float2(vx, vy);
+#else
+                if (out) __stcs(reinterpret_cast<float2 *>(out + (size_t)j * kM + 2 * tid), make_float2(vx, vy));   // written once, not re-read here
+#endif
 #endif
                 ssum2 = fma2p(acc[j], acc[j], ssum2);
                 smax = fmaxf(smax, fmaxf(fabsf(vx), fabsf(vy)));
@@ -264,23 +254,21 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     float2 *buf1 = buf0 + kStep * kRow;
     float2 *stw = buf1 + kStep * kRow;                             // [kTwCount]
     float2 *sph = stw + kTwCount;                                  // [K] phasors of this series' STEC trial (a2)
-    float *sred = reinterpret_cast<float *>(sph + kH);             // 16 floats, 16 doubles, the mbarrier
+    float *sred = reinterpret_cast<float *>(sph + kH + 1);         // 16 floats, 16 doubles, the mbarrier
     double *sdred = reinterpret_cast<double *>(sred + 16);
     const uint32_t bar = smem_u32(sdred + 16);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int series = blockIdx.x % a.nseries;
     const int span = blockIdx.x / a.nseries;
-    const long long qs = (long long)span * a.span_len;
-    if (qs >= a.nc) return;
-    const long long qe = (qs + a.span_len < a.nc) ? qs + a.span_len : a.nc;
-    const bool is_last = (qe == a.nc);
+    const int nc = (int)a.nc;                    // slices of the launch (an int at the boundary)
+    const int qs = span * a.span_len;
+    if (qs >= nc) return;
+    const int qe = (qs + a.span_len < nc) ? qs + a.span_len : nc;
+    const bool is_last = (qe == nc);
+    const bool trials = a.zmap_trials != 0;      // the STEC trial phasor multiplies the beam sums on their way in (a2)
 
-    Ctx c;
-    const int zi = a.zmap_trials ? series / a.zmap_trials : series;
-    c.Zs = a.Z + (size_t)zi * a.K * (size_t)a.zpitch;
-    c.ph = a.zmap_trials ? a.Dph + (size_t)(series % a.zmap_trials) * a.K : nullptr;
-    c.zpitch = a.zpitch; c.nc = a.nc; c.K = a.K; c.k0 = a.k0; c.bulk_rows = a.vec_ok; c.tiled = a.ztile;
+    const float2 *Zs = a.Z + (size_t)(trials ? series / a.zmap_trials : series) * a.K * (size_t)a.zpitch;
 
     if (tid == 0) {
         mbar_init(bar, 1);
@@ -288,10 +276,12 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     }
     for (int i = tid; i < kTwCount; i += kThreads) stw[i] = a.tw[i];
     for (int i = tid; i < kStageF2; i += kThreads) stage[i] = make_float2(0.f, 0.f);   // unselected bins stay zero
-    if (c.ph) {
+    if (trials) {
+        const float2 *ph = a.Dph + (size_t)(series % a.zmap_trials) * a.K;
         sph[tid] = make_float2(1.f, 0.f);
+        if (tid == 0) sph[kH] = make_float2(1.f, 0.f);           // the always-zero bin 512
         __syncthreads();
-        for (int i = tid; i < a.K; i += kThreads) sph[a.k0 + i] = c.ph[i];
+        for (int i = tid; i < a.K; i += kThreads) sph[a.k0 + i] = ph[i];
     }
     float2 *stage_k = stage + a.k0 * kStep;      // the copies write rows k0 .. k0 + K - 1
     u64 g[kP];                                   // the 16 tap pairs of residues 2 tid, 2 tid + 1, for the whole span
@@ -309,36 +299,31 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     __syncthreads();                             // mbarrier, twiddles and history visible
 
     // the first step of a span that starts inside the block is a warm-up: transform the 16 slices before it
-    const long long q_first = span == 0 ? qs : qs - kStep;
+    const int q_first = span == 0 ? qs : qs - kStep;
     uint32_t phase = 0;
-    bool async = stage_fill(c, q_first, stage_k, bar, tid);
+    bool async = stage_fill(a, Zs, q_first, stage_k, bar, tid);
 
-    float *out = a.series ? a.series + (size_t)series * a.series_pitch + a.out0 : nullptr;
-    float *yout = a.yout ? a.yout + (size_t)series * a.yout_pitch + a.out0 : nullptr;
     double dsum = 0.0;
-    Emit em;
-    em.cand = a.cand; em.count = a.count; em.cap = a.cap;
-    em.series = (uint32_t)series; em.trial = (uint32_t)(series % a.D);
-    em.thr = a.thr ? a.thr[series] : __int_as_float(0x7f800000);
-    em.sigma = a.thr ? a.sigma_ref[series] : 0.f;
+    const float thr = a.thr ? a.thr[series] : __int_as_float(0x7f800000);    // +inf: no emission from the epilogue
 
-    for (long long q = q_first; q < qe; q += kStep) {
+    for (int q = q_first; q < qe; q += kStep) {
         if (async) { while (!mbar_try_wait(bar, phase)) {} phase ^= 1; }
         else __syncthreads();
 #ifndef LOFAR_ABLATE_FFT
-        if (c.ph) pass_a<true>(stage, sph, cur, stw, tid);
+        if (trials) pass_a<true>(stage, sph, cur, stw, tid);
         else pass_a<false>(stage, sph, cur, stw, tid);
 #endif
         __syncthreads();                         // radix-16 results of all 16 slices in cur, stage free
-        if (q + kStep < qe) async = stage_fill(c, q + kStep, stage_k, bar, tid);   // flies during pass B + FIR
+        if (q + kStep < qe) async = stage_fill(a, Zs, q + kStep, stage_k, bar, tid);   // flies during pass B + FIR
 #ifndef LOFAR_ABLATE_FFT
         fft512_pass_b<false>(cur + warp * kRow, stw, lane);
 #endif
         __syncthreads();
 
-        if (q >= qs && yout) {
+        if (q >= qs && a.yout) {
             // LSMR inversion (f1): hand the inverse-DFT rows to the solver instead of applying the matched FIR
-            const int nvalid = (qe - q < kStep) ? (int)(qe - q) : kStep;
+            float *yout = a.yout + (size_t)series * a.yout_pitch + a.out0;
+            const int nvalid = (qe - q < kStep) ? qe - q : kStep;
             for (int j = 0; j < nvalid; ++j)
                 *reinterpret_cast<float2 *>(yout + (size_t)(q + j) * kM + 2 * tid) = cur[j * kRow + pn];
             if (is_last && q + kStep >= qe) {
@@ -351,18 +336,17 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
             }
             __syncthreads();
         } else if (q >= qs) {
-            const int nvalid = (qe - q < kStep) ? (int)(qe - q) : kStep;
+            const int nvalid = (qe - q < kStep) ? qe - q : kStep;
             u64 ssum2 = 0ull;
             float smax = 0.f;
-            float *o = out ? out + (size_t)q * kM : nullptr;
-            em.sample0 = a.offset + (uint64_t)a.out0 + (uint64_t)q * kM;
+            float *o = a.series ? a.series + (size_t)series * a.series_pitch + a.out0 + (size_t)q * kM : nullptr;
 #ifndef LOFAR_ABLATE_FIR
             if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
             else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
 #endif
-            if (smax > em.thr)
-                emit_step(prev, cur, a.gs, tid, pn, nvalid, em.cand, em.count, em.cap, em.series, em.trial, em.thr, em.sigma,
-                          em.sample0);
+            if (smax > thr)
+                emit_step(prev, cur, a.gs, tid, pn, nvalid, a.cand, a.count, a.cap, (uint32_t)series, (uint32_t)(series % a.D),
+                          thr, a.sigma_ref[series], a.offset + (uint64_t)a.out0 + (uint64_t)q * kM);
             dsum += (double)(LO(ssum2) + HI(ssum2));
 #pragma unroll
             for (int s = 16; s > 0; s >>= 1) smax = fmaxf(smax, __shfl_xor_sync(0xffffffffu, smax, s));
@@ -447,6 +431,7 @@ __global__ void __launch_bounds__(kThreads, 1) rescan_kernel(RescanArgs r)
     for (int i = tid; i < kTwCount; i += kThreads) stw[i] = r.tw[i];
     for (int i = tid; i < kStageF2; i += kThreads) stage[i] = make_float2(0.f, 0.f);
     sph[tid] = make_float2(1.f, 0.f);
+    if (tid == 0) sph[kH] = make_float2(1.f, 0.f);
     float2 *stage_k = stage + r.k0 * kStep;
     u64 g[kP];
 #pragma unroll
@@ -484,17 +469,13 @@ __global__ void __launch_bounds__(kThreads, 1) rescan_kernel(RescanArgs r)
             __syncthreads();
             fft512_pass_b<false>(buf1 + warp * kRow, stw, lane);
             __syncthreads();
-            Emit em;
-            em.cand = r.cand; em.count = r.count; em.cap = r.cap;
-            em.series = (uint32_t)series; em.trial = (uint32_t)d; em.thr = thr; em.sigma = sig;
-            em.sample0 = r.offset + (uint64_t)q * kM;
             const int nvalid = (r.T - q < kStep) ? (int)(r.T - q) : kStep;
             u64 ssum2 = 0ull;
             float smax = 0.f;
             fir_step<false>(buf0, buf1, g, pn, nullptr, tid, nvalid, ssum2, smax);
-            if (smax > em.thr)
-                emit_step(buf0, buf1, r.gs, tid, pn, nvalid, em.cand, em.count, em.cap, em.series, em.trial, em.thr, em.sigma,
-                          em.sample0);
+            if (smax > thr)
+                emit_step(buf0, buf1, r.gs, tid, pn, nvalid, r.cand, r.count, r.cap, (uint32_t)series, (uint32_t)d, thr, sig,
+                          r.offset + (uint64_t)q * kM);
             __syncthreads();
         }
     }

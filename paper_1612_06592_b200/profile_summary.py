@@ -58,6 +58,57 @@ def read_raw(rep: str):
     return res
 
 
+def phases(rep: str, kernel: str, min_share: float = 0.01):
+    """Warp-stall samples of `kernel` from the source page of the capture (ncu -i ... --page source --csv), summed over
+    the stretches of SASS between barriers (BAR / SYNCS / EXIT): one row per stretch with its share of the samples, the
+    warp instructions executed, the most frequent opcodes and the most frequent stall reasons."""
+    out = subprocess.run(["ncu", "-i", rep, "--page", "source", "--csv", "--kernel-name", f"regex:{kernel}"],
+                         capture_output=True, text=True).stdout
+    rows = list(csv.reader(io.StringIO(out)))
+    start = next((i for i, r in enumerate(rows) if r and r[0] == "Address"), None)
+    if start is None:
+        return []
+    hdr = rows[start]
+    ix = {h: i for i, h in enumerate(hdr)}
+    stalls = [h for h in hdr if h.startswith("stall_") and "Not Issued" not in h]
+    data = []
+    for r in rows[start + 1:]:
+        if len(r) != len(hdr) or r[0] == "Address":
+            break                                   # the next launch of the same kernel
+        data.append(r)
+    total = sum(int(r[ix["# Samples"]] or 0) for r in data) or 1
+    segs, cur = [], None
+
+    def new(i):
+        return {"first": i, "samples": 0, "exec": 0, "ops": {}, "stalls": {}}
+    cur = new(0)
+    for i, r in enumerate(data):
+        words = r[ix["Source"]].split()
+        op = words[1] if words and words[0].startswith("@") and len(words) > 1 else (words[0] if words else "")
+        cur["samples"] += int(r[ix["# Samples"]] or 0)
+        e = int(r[ix["Instructions Executed"]] or 0)
+        cur["exec"] += e
+        cur["ops"][op.split(".")[0]] = cur["ops"].get(op.split(".")[0], 0) + e
+        for st in stalls:
+            cur["stalls"][st[6:]] = cur["stalls"].get(st[6:], 0) + int(r[ix[st]] or 0)
+        if op.startswith(("BAR", "SYNCS", "EXIT")):
+            cur["last"] = i
+            segs.append(cur)
+            cur = new(i + 1)
+    cur["last"] = len(data) - 1
+    segs.append(cur)
+    res = []
+    for sg in segs:
+        if sg["samples"] / total < min_share:
+            continue
+        top = sorted(sg["ops"].items(), key=lambda x: -x[1])[:5]
+        st = sorted(sg["stalls"].items(), key=lambda x: -x[1])[:4]
+        res.append({"sass": f"{sg['first']}-{sg['last']}", "share": sg["samples"] / total, "warp_instr": sg["exec"],
+                    "top_ops": ", ".join(f"{k} {v / 1e6:.0f}M" for k, v in top if v),
+                    "top_stalls": ", ".join(f"{k} {v / max(1, sg['samples']):.0%}" for k, v in st if v)})
+    return res
+
+
 def to_bytes(v, unit):
     mult = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}.get(unit, 1.0)
     return None if v is None else v * mult
@@ -71,6 +122,7 @@ def main():
     ap.add_argument("--json", default=os.path.join("profiles", "ncu_summary.json"))
     ap.add_argument("--md", default=None)
     ap.add_argument("--command", default="", help="the command line that made the capture (recorded in the summary)")
+    ap.add_argument("--phases", default="", help="kernel name (regex) whose warp-stall samples are split at its barriers")
     args = ap.parse_args()
     bench = json.loads(open(args.bench).read().strip().splitlines()[-1])
     cfg = re.match(r"(configs\[\d\])", bench["config"]["workload"]).group(1)
@@ -102,6 +154,15 @@ def main():
             lines.append(f"{k['name']}: DRAM traffic {e['dram_GB_per_launch']:.3f} GB per launch vs "
                          f"{e['algorithmic_GB_per_launch']:.3f} GB algorithmic (ratio "
                          f"{e['dram_GB_per_launch'] / e['algorithmic_GB_per_launch']:.3f}); busiest unit: {e['limiter']}.")
+    if args.phases:
+        ph = phases(args.rep, args.phases)
+        if ph:
+            lines += ["", f"{args.phases}: warp-stall samples between barriers (source page of the same capture, first "
+                          "launch; SASS line ranges of this build):", "",
+                      "| SASS lines | share of samples | warp instructions | most executed opcodes | top stall reasons |",
+                      "|---|---|---|---|---|"]
+            lines += [f"| {p['sass']} | {p['share']:.1%} | {p['warp_instr'] / 1e6:.1f} M | {p['top_ops']} | {p['top_stalls']} |"
+                      for p in ph]
     os.makedirs(os.path.dirname(args.json) or ".", exist_ok=True)
     json.dump(summary, open(args.json, "w"), indent=1, sort_keys=True)
     md = args.md or os.path.join("profiles", f"{args.tag}_ncu_full.md")

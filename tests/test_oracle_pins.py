@@ -433,3 +433,13 @@ def test_config0_timedomain_generator_small(oracle):
     # carrier, so noise can move the largest lobe by one carrier period
     assert abs(int(np.argmax(np.abs(series[pl.beam]))) - n_inj) <= 4
     assert np.abs(series[pl.beam]).max() > 0.6 * 2 * w.S * pl.amp
+
+
+def test_golden_values_are_regenerated_by_the_committed_script():
+    """tests/golden/make_ppf_pins.py (numpy / scipy only, no oracle code) reproduces every stored number."""
+    import importlib.util
+    path = os.path.join(os.path.dirname(__file__), "golden", "make_ppf_pins.py")
+    spec = importlib.util.spec_from_file_location("make_ppf_pins", path)
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    assert mod.main() == 0
