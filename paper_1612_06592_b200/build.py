@@ -7,8 +7,7 @@ Ablation builds (the measurements DESIGN.md section 8 quotes): `--define NAME [-
 variant with -DNAME into PATH (objects under build/<names>/); run it with LOFAR_MOON_LIB=PATH, which the binding
 honours. Switches: LOFAR_FIR_PACKED (synthesis FIR with packed FFMA2 instead of scalar FFMA), LOFAR_FFT_SCALAR (the
 transform's complex adds / butterflies as scalar pairs instead of FADD2 / FFMA2), LOFAR_ST_PLAIN (series stores with
-the default cache policy instead of st.global.cs), LOFAR_PB_OLDLD / LOFAR_PB_OLDST (radix-32 pass with pad() evaluated
-per access), LOFAR_ABLATE_STORES
+the default cache policy instead of st.global.cs), LOFAR_ABLATE_STORES
 (inverse PPF without its series stores), LOFAR_ABLATE_FIR (no FIR arithmetic), LOFAR_ABLATE_FFT (no transform
 arithmetic). Ablated variants compute wrong results by design; they exist to attribute time.
 """

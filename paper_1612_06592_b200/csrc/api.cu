@@ -272,10 +272,16 @@ lofar_status build(lofar_plan *p)
         for (int n = 0; n < kHalf; ++n)
             gs[(size_t)t * kHalf + n] = make_float2((float)(kMfft * p->h[2 * n + kMfft * t]),
                                                     (float)(kMfft * p->h[2 * n + 1 + kMfft * t]));
-    // twiddles: w1024[256] for the pre-pass, TB[r][j] = exp(2 pi i j r / 512) (r < 32, j < 16) for the radix-32 pass
+    // twiddles: w1024[256] for the pre-pass, TBs[r][j] = +-exp(2 pi i j r / 512) (r < 32, j < 16) for the radix-32 pass
     for (int m = 0; m < 256; ++m) tw[m] = unit_phasor((double)m / 1024.0);
+    // the odd rows carry the sign (-1)^((r-1)/2): it rotates the odd half of the radix-32 butterflies by 8 outputs, which
+    // lets the two lanes of a butterfly exchange half as many registers (fft_warp.cuh: fft512_pass_b)
     for (int r = 0; r < 32; ++r)
-        for (int jj = 0; jj < 16; ++jj) tw[256 + r * 16 + jj] = unit_phasor((double)(jj * r) / 512.0);
+        for (int jj = 0; jj < 16; ++jj) {
+            float2 v = unit_phasor((double)(jj * r) / 512.0);
+            if ((r & 3) == 3) { v.x = -v.x; v.y = -v.y; }
+            tw[256 + r * 16 + jj] = v;
+        }
 
     lofar_status st;
     if ((st = dev_alloc(p, &p->dW, L.W)) != LOFAR_OK) return st;

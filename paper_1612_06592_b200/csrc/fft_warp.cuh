@@ -77,18 +77,20 @@ __device__ __forceinline__ void idft16p(u64 *x)
 
 // Radix-32 pass of the 512-point inverse FFT (512 = 16 x 32) of one slice row by one warp, in place. The row holds
 // the radix-16 results at 16 j + m. Butterfly j (0..15) is a 32-point DFT of elements j + 16 r with twiddles
-// exp(2 pi i j r / 512) (TW: applied here on load; otherwise the producer of the row has applied them);
-// lanes j and j + 16 share it: each does the 16-point DFT of the even / odd r, the odd lane applies W32^m, the
-// halves are exchanged with shuffles; outputs go to j + 16 m (m < 16 low lane, m >= 16 high).
+// TB[r][j] = exp(2 pi i j r / 512) (TW: applied here on load; otherwise the producer of the row has applied them);
+// lanes j and j + 16 share it: the low lane does the 16-point DFT E of the even r, the high lane that of the odd r, O.
+// The table carries a factor (-1)^((r-1)/2) on its odd rows (TBs, built in api.cu): the inputs of the high lane
+// arrive as (-1)^r' x[r'], which rotates its outputs by 8 -- register i holds O[(i + 8) mod 16] -- so that both
+// lanes can hand over the SAME registers 8..15 (E[8..15] one way, W32^i O[i] the other) in 8 exchanges instead of 16:
+// the low lane finishes outputs i and 16 + i, the high lane 8 + i and 24 + i (i < 8); output m goes to j + 16 m.
 template <bool TW>
 __device__ __forceinline__ void fft512_pass_b(float2 *row, const float2 *stw, int lane)
 {
     u64 x[16];
-    // pad(lane + 32 r) = lane + (lane >> 4) + 34 r: one base pointer and compile-time offsets (the compiler does not
-    // fold the shift inside pad() by itself and would spend three integer instructions per access)
+    // pad(lane + 32 r) = lane + (lane >> 4) + 34 r: one base pointer and compile-time offsets
     const float2 *src = row + lane + (lane >> 4);
     if (TW) {
-        const float2 *T = stw + 256 + lane;      // T[32 r' + lane] = exp(2 pi i j (hh + 2 r') / 512)
+        const float2 *T = stw + 256 + lane;      // T[32 r' + lane] = TBs[2 r' + hh][lane & 15]
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
             const float2 t = T[32 * r];
@@ -96,16 +98,12 @@ __device__ __forceinline__ void fft512_pass_b(float2 *row, const float2 *stw, in
         }
     } else {
 #pragma unroll
-#ifdef LOFAR_PB_OLDLD
-        for (int r = 0; r < 16; ++r) x[r] = lds64(row + pad(lane + 32 * r));
-#else
         for (int r = 0; r < 16; ++r) x[r] = lds64(src + 34 * r);
-#endif
     }
     idft16p(x);
     const bool hi = lane >= 16;
     if (hi) {
-        // W32^m = exp(2 pi i m / 32), m = 0..15
+        // register i holds O[k], k = (i + 8) mod 16: times W32^k = exp(2 pi i k / 32)
         const float c[16] = {1.f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
                              0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
                              0.19509032201612826785f, 0.f, -0.19509032201612826785f, -0.38268343236508977173f,
@@ -117,24 +115,31 @@ __device__ __forceinline__ void fft512_pass_b(float2 *row, const float2 *stw, in
                               0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
                               0.38268343236508977173f, 0.19509032201612826785f};
 #pragma unroll
-        for (int m = 1; m < 16; ++m) x[m] = cmulp(x[m], c[m], sn[m]);
+        for (int i = 0; i < 16; ++i) {
+            const int k = (i + 8) & 15;
+            if (k) x[i] = cmulp(x[i], c[k], sn[k]);
+        }
     }
-    // low lane: E + O', high lane: E - O'  ==  other + sg * own with sg = +1 / -1
+    // low lane: own = E[i], received = W32^i O[i]; high lane: own = W32^(8+i) O[8+i], received = E[8+i]
     const u64 sg = hi ? PK(-1.f, -1.f) : PK(1.f, 1.f);
+    __syncwarp();
+    const int jl = lane & 15;
+    float2 *dsum = row + jl + (hi ? 17 * 8 : 0);               // outputs i (low) / 8 + i (high): pad(j + 16 m) = j + 17 m
+    float2 *ddif = row + jl + (hi ? 17 * 24 : 17 * 16);        // outputs 16 + i (low) / 24 + i (high)
 #pragma unroll
-    for (int m = 0; m < 16; ++m) {
-        const u64 other = __shfl_xor_sync(0xffffffffu, x[m], 16);
-        x[m] = fma2(x[m], sg, other);
+    for (int i = 0; i < 8; ++i) {
+        const u64 other = __shfl_xor_sync(0xffffffffu, x[8 + i], 16);
+        const u64 s2 = add2(x[i], other);                      // E + W O on either lane
+        const u64 d2 = sub2(x[i], other);                      // low: E - W O;  high: W O - E
+        x[i] = s2;
+        x[8 + i] = fma2(d2, sg, 0ull);
     }
     __syncwarp();
-    // pad(base + 16 m) = base + (base >> 4) + 17 m with base = (lane & 15) + (hi ? 256 : 0)
-    float2 *dst = row + (lane & 15) + (hi ? 256 + 16 : 0);
 #pragma unroll
-#ifdef LOFAR_PB_OLDST
-    for (int m = 0; m < 16; ++m) sts64(row + pad((lane & 15) + (hi ? 256 : 0) + 16 * m), x[m]);
-#else
-    for (int m = 0; m < 16; ++m) sts64(dst + 17 * m, x[m]);
-#endif
+    for (int i = 0; i < 8; ++i) {
+        sts64(dsum + 17 * i, x[i]);
+        sts64(ddif + 17 * i, x[8 + i]);
+    }
     __syncwarp();
 }
 

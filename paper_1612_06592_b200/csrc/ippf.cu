@@ -9,9 +9,11 @@
 //              shared-memory stage by bulk asynchronous copies (cp.async.bulk + mbarrier; one copy of
 //              K*128 bytes from the plan's tiled scratch, one copy per row from a caller's Z), issued one
 //              step ahead so that they fly during the FFT and FIR of the current step;
-//   pre-pass : reads the stage, applies the trial phasor if asked, builds the packed half-spectrum V
-//              (fft_math.cuh) and stores it transposed -- slice-major -- into the current slice buffer;
-//   FFT      : warp w transforms slice w in place: a radix-16 and a radix-32 pass (fft512_warp);
+//   pass A   : thread (bin residue j mod 32, slice t) reads its 16 bins j + 32 r and their mirrors from the stage,
+//              applies the trial phasor if asked, forms the packed half-spectrum V of the real transform
+//              (fft_math.cuh), does the radix-16 butterflies over r, applies the radix-32 twiddles and stores the
+//              result slice-major into the current slice buffer (V itself is never written);
+//   pass B   : warp w finishes slice w in place: the radix-32 pass of 512 = 16 x 32 (fft512_pass_b);
 //   FIR      : thread n owns output residues r = 2n, 2n+1 and keeps their 16 tap pairs in registers; the
 //              31-slice window (15 carried + 16 new) is read from the previous and current slice buffers;
 //              16 x 1024 contiguous output samples are written per step.
@@ -155,8 +157,9 @@ __device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, f
         }
     }
     idft16p(x);
-    const float2 *T = stw + 256 + 16 * j;          // T[m] = exp(2 pi i j m / 512)
+    const float2 *T = stw + 256 + 16 * j;          // T[m] = TBs[j][m] = +-exp(2 pi i j m / 512), minus for j = 3 (mod 4)
     float2 *row = dst + t * kRow + 17 * j;         // pad(16 j + m) = 17 j + m
+    if ((j & 3) == 3) x[0] = PK(-LO(x[0]), -HI(x[0]));      // TBs[j][0] = -1: the one twiddle that is not loaded
     sts64(row, x[0]);
 #pragma unroll
     for (int m = 1; m < 16; ++m) {
