@@ -403,6 +403,22 @@ def run_gpu(args, idx=None):
                         "launching stream inside the timed region (K*8 B read + 4096 B written per series-slice "
                         "for ippf_kernel; 2*S*2*esize B read + B*8 B written per (sub-band, slice) for beamform). "
                         "`bound` names the roofline the kernel is designed against; `limiter` is what ncu shows."}
+    # The same kernel against the fp32 pipe (configs 2-4 are predicted ALU-bound): flop per (series, slice)
+    # of the inverse PPF = 512-point complex FFT, 5 N log2 N = 23040 (the usual count, twiddles included) + pair pre-pass
+    # 8 flop x 256 pairs = 2048 + FIR 2 x 16 taps x 1024 = 32768 -> 57856; peak = SMs x 128 FMA lanes x 2 flop x the SM
+    # clock sampled during the timed region.
+    if dom["kernel"] == "ippf_kernel":
+        sms = torch.cuda.get_device_properties(local).multi_processor_count
+        mhz = (clocks or {}).get("sm_mhz") or 1965.0
+        flop = 57856.0 * ninv * w.T / dom["launches_per_step"]
+        if mode in ("lsmr",):
+            flop -= 32768.0 * ninv * w.T / dom["launches_per_step"]          # no FIR in the kernel: LSMR solves instead
+        peak_tf = sms * 128 * 2 * mhz * 1e6 / 1e12
+        ach_tf = flop / (dom["ms_per_launch"] * 1e-3) / 1e12
+        roofline["alu"] = {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach_tf / peak_tf,
+                           "flop_per_series_slice": 57856,
+                           "note": "fp32 pipe: SMs x 128 lanes x 2 flop x sampled SM clock; what ncu names as the busiest "
+                                   "units is in `limiter`"}
     chain = {"algorithmic_GB_per_step": chain_bytes / 1e9,
              "achieved_GBps": chain_bytes / 1e9 / (ms_step * 1e-3),
              "frac_of_peak": chain_bytes / 1e9 / (ms_step * 1e-3) / peak,
