@@ -501,7 +501,7 @@ def main():
     ap.add_argument("--overlap", action="store_true",
                     help="lofar_plan_set_overlap(1): beamformer of chunk c+1 beside the inverse PPF of chunk c")
     ap.add_argument("--overlap-chunk", type=int, default=0, help="slices per pipeline chunk (0 = library default)")
-    ap.add_argument("--scratch-mb", type=int, default=0, help="lofar_plan_set_scratch_limit in MiB (0 = default 4 GiB)")
+    ap.add_argument("--scratch-mb", type=int, default=0, help="lofar_plan_set_scratch_limit in MiB (0 = default 16 GiB)")
     ap.add_argument("--compare-cufft", action="store_true", help="also time cuFFT C2R (via torch) as a comparison for a3")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "gpu":

@@ -164,7 +164,7 @@ LOFAR_API lofar_status lofar_plan_workspace_bytes(lofar_plan *plan, size_t *byte
  * only memory the plan takes elsewhere is 256 bytes of pinned HOST memory for streaming counts. */
 LOFAR_API lofar_status lofar_plan_set_allocator(lofar_plan *plan, void *(*alloc)(size_t, void *),
                                                 void (*free_)(void *, void *), void *ctx);
-/* Upper bound in bytes for the beam-sum scratch (default 4 GiB; all slots together).  A block longer
+/* Upper bound in bytes for the beam-sum scratch (default 16 GiB -- one chunk for a 0.67 s block of 24 beams x 488 sub-bands; all slots together).  A block longer
  * than the chunk is processed chunk by chunk, history handed over on the device. */
 LOFAR_API lofar_status lofar_plan_set_scratch_limit(lofar_plan *plan, size_t bytes);
 /* Two-lane block pipeline of lofar_run_block / lofar_stream_push (step a6 applied inside a block: the "CUDA

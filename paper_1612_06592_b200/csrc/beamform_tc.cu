@@ -11,7 +11,7 @@
 // compute-bound at the largest beam count: profiles/r1_b shows the SIMT kernel at 70 % issue / 50 %
 // FMA-pipe utilisation and 24 % of DRAM bandwidth for 24 beams.
 //
-// CTA = 128 threads, one sub-band, a run of 128-slice tiles.  Per tile: 96..128 threads each load
+// CTA = 128 threads, one sub-band, a run of 8 128-slice tiles.  Per tile: 96..128 threads each load
 // 8 (station,pol) rows x 16 bytes, add the polarisations, convert to fp16 and write one 8x16-byte core
 // matrix of the K-major no-swizzle operand layout; one thread issues the MMAs (kind::f16, M=128,
 // N=2B padded to 16, K=16 per instruction) and commits to an mbarrier; the four warps read their 32
@@ -267,7 +267,13 @@ int launch_beamform_tc(const BeamformArgs &b, const void *wimg, cudaStream_t st)
     a.img16 = (int)(tc_image_halfs(b.S, b.B) * 2 / 16);
     a.wimg = static_cast<const uint4 *>(wimg);
     const long long tiles = (b.nt + 127) / 128;
-    a.tiles_per_cta = tiles < 32 ? (int)tiles : 32;
+    // 8 tiles (1024 slices) per CTA: measured optimum on B200 for configs[2] (ms per block for 1 / 2 / 4 / 8 / 16 / 32 / 88
+    // tiles: 5.09 / 3.68 / 3.30 / 3.22 / 3.34 / 3.45 / 3.81) -- long enough to amortise the per-CTA prologue (weight
+    // images, TMEM allocation), short enough that the CTAs in flight write a narrow band of Z tiles
+#ifndef LOFAR_BF_TILES
+#define LOFAR_BF_TILES 8
+#endif
+    a.tiles_per_cta = tiles < LOFAR_BF_TILES ? (int)tiles : LOFAR_BF_TILES;
     dim3 grid((unsigned)b.K, (unsigned)((tiles + a.tiles_per_cta - 1) / a.tiles_per_cta));
     const size_t smem = (size_t)a.kchunks * kLboA + 2 * (size_t)a.img16 * 16 + 16;
     beamform_tc_kernel<<<grid, kTcThreads, smem, st>>>(a);

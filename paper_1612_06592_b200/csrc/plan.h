@@ -167,7 +167,7 @@ struct lofar_plan {
     void *(*alloc_fn)(size_t, void *) = nullptr;
     void (*free_fn)(void *, void *) = nullptr;
     void *alloc_ctx = nullptr;
-    size_t scratch_limit = (size_t)4 << 30;   // bytes of beam-sum scratch (all slots together)
+    size_t scratch_limit = (size_t)16 << 30;  // bytes of beam-sum scratch (all slots together); sized for 180 GB of HBM
     // Two-lane block pipeline (lofar_plan_set_overlap): the beamformer of chunk c+1 runs on a low-priority stream
     // beside the inverse PPF of chunk c, on the SMs the inverse PPF leaves free; two scratch slots.
     int overlap = 0;                   // requested: 0 = serial (default: measured faster), 1 = pipeline

@@ -109,7 +109,7 @@ def test_capacity_is_a_state_error(torch):
 @pytest.mark.parametrize("T,limit_slices", [(200, 64), (136, 32), (96, 96)])
 def test_scratch_chunks_hand_over_history(torch, oracle, T, limit_slices):
     """A reduced scratch limit forces lofar_run_block through several time chunks (the path configs[2] takes
-    at full size: 131072 slices = three chunks of the 4 GiB default): out0 / step0 offsets, scratch reuse and
+    at full size: 195312 slices = two chunks of the 16 GiB default): out0 / step0 offsets, scratch reuse and
     the ping-pong history hand-over between the launches."""
     w, tau, X = _case(S=4, B=5, K=24, k0=200, T=T, dtype="ci8", kappa=4.0, n_pulses=2)
     pipe = oracle.OraclePipeline(tau=tau, stec=np.asarray(w.stec), K=w.K, k0=w.k0, kappa=w.kappa)
