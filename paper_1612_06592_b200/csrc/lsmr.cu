@@ -8,7 +8,8 @@
 //     (A^T u)[n] = sum_{t<16} taps[t][r] u[n - t],   n = 0 .. n_un-1   (n_un = n_eq + 15 unknown slices)
 // with b = y / 1024.  Every (series, residue) runs the LSMR recurrences with its own scalars; nothing couples
 // them, so the vectors are laid out [row][1024] and a thread owns one residue of a run of rows: loads are
-// coalesced over residues and the 16-tap window slides through registers along the rows.
+// coalesced over residues and the 16-tap window slides through registers along the rows, 16 rows at a time with all
+// loads of a group issued before its arithmetic (the solver is a stream of 13 vector passes per iteration).
 // Vectors are kept unnormalised (u', v') next to their norms (beta, alpha): a pass never has to wait for a norm
 // it produces itself.  Norms: per-chunk partial sums in double, added in a fixed order.
 #include "plan.h"
@@ -30,7 +31,9 @@ __device__ __forceinline__ double safe_div(double a, double d) { return d != 0.0
 
 // u'[m] = sum_t taps[t] v'[m+t] / alpha - alpha * u'[m] / beta_old    (first = 0)
 // or first = 1:  u' = b / 1024 (the right-hand side), nothing else.
-__global__ void __launch_bounds__(kLsmrThreads) u_kernel(float *u, long long upitch, long long n_eq, const float *v,
+// 4 (u) and 3 (v) CTAs per SM: measured optimum on B200 (1 / 2 / 4 / 6 for u: 872 / 887 / 784 / 1165 ms per configs[2] block of
+// 25 iterations; more spills, fewer leaves too few loads in flight)
+__global__ void __launch_bounds__(kLsmrThreads, 4) u_kernel(float *u, long long upitch, long long n_eq, const float *v,
                                                          long long vpitch, const float *gs, const Scal *sc, double *partial,
                                                          int nchunks, int first)
 {
@@ -48,28 +51,42 @@ __global__ void __launch_bounds__(kLsmrThreads) u_kernel(float *u, long long upi
         const Scal z = sc[(size_t)series * kRes + r];
         const float ia = (float)z.inv_alpha, ab = (float)(z.alpha * z.inv_beta);
         const float *pv = v + (size_t)series * vpitch + r;
-        float tap[kTapsN], win[kTapsN];
+        // rows in groups of 16: the 16 new rows of v' and the 16 rows of u' are loaded before anything is computed (32
+        // independent loads per thread in flight -- the kernel is a stream and lives on memory-level parallelism); the
+        // window w[0..30] = v'[mb .. mb+30] slides by 16 registers per group
+        float tap[kTapsN], w[2 * kTapsN - 1];
 #pragma unroll
         for (int t = 0; t < kTapsN; ++t) tap[t] = gs[t * kRes + r] * (1.0f / 1024.0f);
 #pragma unroll
-        for (int t = 0; t < kTapsN - 1; ++t) win[t + 1] = pv[(size_t)(m0 + t) * kRes];
-        for (long long m = m0; m < m1; ++m) {
+        for (int t = 0; t < kTapsN - 1; ++t) w[t] = pv[(size_t)(m0 + t) * kRes];
+        for (long long mb = m0; mb < m1; mb += kTapsN) {
+            float un[kTapsN];
 #pragma unroll
-            for (int t = 0; t < kTapsN - 1; ++t) win[t] = win[t + 1];
-            win[kTapsN - 1] = pv[(size_t)(m + kTapsN - 1) * kRes];        // rows m .. m+15 of v' (n_un = n_eq + 15)
-            float acc = 0.f;
+            for (int k = 0; k < kTapsN; ++k) {
+                const bool ok = mb + k < m1;                     // rows m .. m+15 of v' exist for m < n_eq (n_un = n_eq + 15)
+                w[kTapsN - 1 + k] = ok ? pv[(size_t)(mb + k + kTapsN - 1) * kRes] : 0.f;
+                un[k] = ok ? pu[(size_t)(mb + k) * kRes] : 0.f;
+            }
 #pragma unroll
-            for (int t = 0; t < kTapsN; ++t) acc = fmaf(tap[t], win[t], acc);
-            const float val = fmaf(acc, ia, -ab * pu[(size_t)m * kRes]);
-            pu[(size_t)m * kRes] = val;
-            s += (double)val * val;
+            for (int k = 0; k < kTapsN; ++k) {
+                float acc = 0.f;
+#pragma unroll
+                for (int t = 0; t < kTapsN; ++t) acc = fmaf(tap[t], w[k + t], acc);
+                const float val = fmaf(acc, ia, -ab * un[k]);
+                if (mb + k < m1) {
+                    pu[(size_t)(mb + k) * kRes] = val;
+                    s += (double)val * val;
+                }
+            }
+#pragma unroll
+            for (int t = 0; t < kTapsN - 1; ++t) w[t] = w[t + kTapsN];
         }
     }
     partial[((size_t)series * nchunks + chunk) * kRes + r] = s;
 }
 
 // v'[n] = sum_t taps[t] u'[n-t] / beta - beta * v'[n] / alpha_old     (first: no second term)
-__global__ void __launch_bounds__(kLsmrThreads) v_kernel(float *v, long long vpitch, long long n_un, const float *u,
+__global__ void __launch_bounds__(kLsmrThreads, 3) v_kernel(float *v, long long vpitch, long long n_un, const float *u,
                                                          long long upitch, long long n_eq, const float *gs, const Scal *sc,
                                                          double *partial, int nchunks, int first)
 {
@@ -79,26 +96,38 @@ __global__ void __launch_bounds__(kLsmrThreads) v_kernel(float *v, long long vpi
     const long long n0 = (long long)chunk * kRows, n1 = n0 + kRows < n_un ? n0 + kRows : n_un;
     const Scal z = sc[(size_t)series * kRes + r];
     const float ib = (float)z.inv_beta, ba = first ? 0.f : (float)(z.beta * z.inv_alpha);
-    float tap[kTapsN], win[kTapsN];       // win[t] = u'[n - t]
+    // as u_kernel: groups of 16 rows, loads first. w[j] = u'[nb - 15 + j], j = 0..30 (zero outside 0 .. n_eq-1)
+    float tap[kTapsN], w[2 * kTapsN - 1];
 #pragma unroll
     for (int t = 0; t < kTapsN; ++t) tap[t] = gs[t * kRes + r] * (1.0f / 1024.0f);
 #pragma unroll
-    for (int t = 0; t < kTapsN - 1; ++t) {
-        const long long m = n0 - 1 - t;
-        win[t] = (m >= 0 && m < n_eq) ? pu[(size_t)m * kRes] : 0.f;
+    for (int j = 0; j < kTapsN - 1; ++j) {
+        const long long m = n0 - (kTapsN - 1) + j;
+        w[j] = (m >= 0 && m < n_eq) ? pu[(size_t)m * kRes] : 0.f;
     }
     double s = 0.0;
-    for (long long n = n0; n < n1; ++n) {
+    for (long long nb = n0; nb < n1; nb += kTapsN) {
+        float vo[kTapsN];
 #pragma unroll
-        for (int t = kTapsN - 1; t > 0; --t) win[t] = win[t - 1];
-        win[0] = n < n_eq ? pu[(size_t)n * kRes] : 0.f;
-        float acc = 0.f;
+        for (int k = 0; k < kTapsN; ++k) {
+            const long long n = nb + k;
+            w[kTapsN - 1 + k] = (n < n1 && n < n_eq) ? pu[(size_t)n * kRes] : 0.f;
+            vo[k] = (!first && n < n1) ? pv[(size_t)n * kRes] : 0.f;
+        }
 #pragma unroll
-        for (int t = 0; t < kTapsN; ++t) acc = fmaf(tap[t], win[t], acc);
-        float val = acc * ib;
-        if (!first) val = fmaf(-ba, pv[(size_t)n * kRes], val);
-        pv[(size_t)n * kRes] = val;
-        s += (double)val * val;
+        for (int k = 0; k < kTapsN; ++k) {
+            float acc = 0.f;
+#pragma unroll
+            for (int t = 0; t < kTapsN; ++t) acc = fmaf(tap[t], w[kTapsN - 1 + k - t], acc);    // u'[n - t]
+            float val = acc * ib;
+            if (!first) val = fmaf(-ba, vo[k], val);
+            if (nb + k < n1) {
+                pv[(size_t)(nb + k) * kRes] = val;
+                s += (double)val * val;
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < kTapsN - 1; ++j) w[j] = w[j + kTapsN];
     }
     partial[((size_t)series * nchunks + chunk) * kRes + r] = s;
 }
@@ -152,15 +181,27 @@ __global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, 
     const float ia = (float)z.inv_alpha, ch = (float)z.ch, cx = (float)z.cx, cv = (float)z.cv;
     const size_t base = (size_t)series * pitch + r;
     const long long n0 = (long long)chunk * kRows, n1 = n0 + kRows < n_un ? n0 + kRows : n_un;
-    for (long long n = n0; n < n1; ++n) {
-        const size_t i = base + (size_t)n * kRes;
-        const float vn = v[i] * ia;
-        if (first) { h[i] = vn; hbar[i] = 0.f; x[i] = 0.f; }
-        else {
-            const float hb = fmaf(-ch, hbar[i], h[i]);
-            hbar[i] = hb;
-            x[i] = fmaf(cx, hb, x[i]);
-            h[i] = fmaf(-cv, h[i], vn);
+    for (long long nb = n0; nb < n1; nb += 4) {
+        float vv[4], hh[4], hb[4], xx[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {                 // loads of four rows first (memory-level parallelism)
+            const bool ok = nb + k < n1;
+            const size_t i = base + (size_t)(nb + k) * kRes;
+            vv[k] = ok ? v[i] : 0.f;
+            if (!first) { hh[k] = ok ? h[i] : 0.f; hb[k] = ok ? hbar[i] : 0.f; xx[k] = ok ? x[i] : 0.f; }
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (nb + k >= n1) break;
+            const size_t i = base + (size_t)(nb + k) * kRes;
+            const float vn = vv[k] * ia;
+            if (first) { h[i] = vn; hbar[i] = 0.f; x[i] = 0.f; }
+            else {
+                const float b = fmaf(-ch, hb[k], hh[k]);
+                hbar[i] = b;
+                x[i] = fmaf(cx, b, xx[k]);
+                h[i] = fmaf(-cv, hh[k], vn);
+            }
         }
     }
 }
