@@ -25,6 +25,7 @@ struct Scal {
     double alpha, beta, alphabar, zetabar, rho, rhobar, cbar, sbar;
     double inv_alpha, inv_beta;          // 1/alpha, 1/beta of the stored (unnormalised) v', u'
     double ch, cx, cv;                   // hbar = h - ch hbar; x += cx hbar; h = v - cv h
+    double cxp;                          // cx of the previous iteration (its x update may still be pending)
 };
 
 __device__ __forceinline__ double safe_div(double a, double d) { return d != 0.0 ? a / d : 0.0; }
@@ -147,7 +148,7 @@ __global__ void __launch_bounds__(kLsmrThreads) scalar_kernel(Scal *sc, const do
         z.alpha = nrm; z.inv_alpha = safe_div(1.0, nrm);
         z.alphabar = z.alpha; z.zetabar = z.alpha * z.beta;
         z.rho = 1.0; z.rhobar = 1.0; z.cbar = 1.0; z.sbar = 0.0;
-        z.ch = 0.0; z.cx = 0.0; z.cv = 0.0;
+        z.ch = 0.0; z.cx = 0.0; z.cv = 0.0; z.cxp = 0.0;
     } else if (which == 2) {
         z.beta = nrm; z.inv_beta = safe_div(1.0, nrm);
     } else {
@@ -165,6 +166,7 @@ __global__ void __launch_bounds__(kLsmrThreads) scalar_kernel(Scal *sc, const do
         z.sbar = safe_div(thetanew, z.rhobar);
         const double zeta = z.cbar * z.zetabar;
         z.zetabar = -z.sbar * z.zetabar;
+        z.cxp = z.cx;
         z.ch = safe_div(thetabar * z.rho, rhoold * rhobarold);
         z.cx = safe_div(zeta, z.rho * z.rhobar);
         z.cv = safe_div(thetanew, z.rho);
@@ -173,12 +175,16 @@ __global__ void __launch_bounds__(kLsmrThreads) scalar_kernel(Scal *sc, const do
 }
 
 // first: h = v'/alpha, hbar = 0, x = 0.   else: hbar = h - ch hbar; x += cx hbar; h = v'/alpha - cv h.
+// xmode (x is only needed after the last iteration, so its update is applied every other iteration and x makes one
+// round trip through HBM instead of two): 0 = this iteration's term now; 1 = defer it (x untouched); 2 = the deferred
+// term of the previous iteration, cxp * hbar_old, then this one -- the same two fused multiply-adds in the same order
+// as two separate updates, so the result is bit-identical.
 __global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, float *x, const float *v, long long pitch,
-                                                         long long n_un, const Scal *sc, int first)
+                                                         long long n_un, const Scal *sc, int first, int xmode)
 {
     const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, series = blockIdx.z;
     const Scal z = sc[(size_t)series * kRes + r];
-    const float ia = (float)z.inv_alpha, ch = (float)z.ch, cx = (float)z.cx, cv = (float)z.cv;
+    const float ia = (float)z.inv_alpha, ch = (float)z.ch, cx = (float)z.cx, cv = (float)z.cv, cxp = (float)z.cxp;
     const size_t base = (size_t)series * pitch + r;
     const long long n0 = (long long)chunk * kRows, n1 = n0 + kRows < n_un ? n0 + kRows : n_un;
     for (long long nb = n0; nb < n1; nb += 4) {
@@ -188,7 +194,10 @@ __global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, 
             const bool ok = nb + k < n1;
             const size_t i = base + (size_t)(nb + k) * kRes;
             vv[k] = ok ? v[i] : 0.f;
-            if (!first) { hh[k] = ok ? h[i] : 0.f; hb[k] = ok ? hbar[i] : 0.f; xx[k] = ok ? x[i] : 0.f; }
+            if (!first) {
+                hh[k] = ok ? h[i] : 0.f; hb[k] = ok ? hbar[i] : 0.f;
+                xx[k] = (ok && xmode != 1) ? x[i] : 0.f;
+            }
         }
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
@@ -199,7 +208,8 @@ __global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, 
             else {
                 const float b = fmaf(-ch, hb[k], hh[k]);
                 hbar[i] = b;
-                x[i] = fmaf(cx, b, xx[k]);
+                if (xmode == 0) x[i] = fmaf(cx, b, xx[k]);
+                else if (xmode == 2) x[i] = fmaf(cx, b, fmaf(cxp, hb[k], xx[k]));
                 h[i] = fmaf(-cv, hh[k], vn);
             }
         }
@@ -238,13 +248,16 @@ int launch_lsmr(float *y, long long ypitch, long long T, float *work, long long 
     scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, ce, 0); ++n;
     v_kernel<<<gu, kLsmrThreads, 0, st>>>(v, wpitch, n_un, y, ypitch, n_eq, gs, sc, partial, cu, 1); ++n;
     scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, cu, 1); ++n;
-    h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 1); ++n;
+    h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 1, 0); ++n;
+    bool pending = false;                               // an x update of the previous iteration is still to be applied
     for (int k = 0; k < iters; ++k) {
         u_kernel<<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 0); ++n;
         scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, ce, 2); ++n;
         v_kernel<<<gu, kLsmrThreads, 0, st>>>(v, wpitch, n_un, y, ypitch, n_eq, gs, sc, partial, cu, 0); ++n;
         scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, cu, 3); ++n;
-        h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 0); ++n;
+        const int xmode = pending ? 2 : (k == iters - 1 ? 0 : 1);
+        h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 0, xmode); ++n;
+        pending = (xmode == 1);
     }
     const dim3 go(kRes / kLsmrThreads, (unsigned)((T + kRows - 1) / kRows), nseries);
     out_kernel<<<go, kLsmrThreads, 0, st>>>(x, wpitch, series, series_pitch, T); ++n;
