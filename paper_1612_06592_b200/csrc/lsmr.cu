@@ -8,7 +8,7 @@
 //     (A^T u)[n] = sum_{t<16} taps[t][r] u[n - t],   n = 0 .. n_un-1   (n_un = n_eq + 15 unknown slices)
 // with b = y / 1024.  Every (series, residue) runs the LSMR recurrences with its own scalars; nothing couples
 // them, so the vectors are laid out [row][1024] and a thread owns one residue of a run of rows: loads are
-// coalesced over residues and the 16-tap window slides through registers along the rows, 16 rows at a time with all
+// coalesced over residues and the 16-tap window slides through registers along the rows, 8 rows at a time with all
 // loads of a group issued before its arithmetic (the solver is a stream of 13 vector passes per iteration).
 // Vectors are kept unnormalised (u', v') next to their norms (beta, alpha): a pass never has to wait for a norm
 // it produces itself.  Norms: per-chunk partial sums in double, added in a fixed order.
@@ -19,6 +19,16 @@ namespace {
 
 constexpr int kTapsN = 16, kRes = 1024, kRows = 64;      // rows per CTA
 constexpr int kLsmrThreads = 256;
+#ifndef LOFAR_LSMR_G
+#define LOFAR_LSMR_G 8
+#endif
+#ifndef LOFAR_U_MINB
+#define LOFAR_U_MINB 4
+#endif
+#ifndef LOFAR_V_MINB
+#define LOFAR_V_MINB 4
+#endif
+constexpr int kG = LOFAR_LSMR_G;           // rows per group: their loads are issued together
 
 // Scalars of one (series, residue), double precision (Fong & Saunders, "Algorithm LSMR", lambda = 0).
 struct Scal {
@@ -32,9 +42,9 @@ __device__ __forceinline__ double safe_div(double a, double d) { return d != 0.0
 
 // u'[m] = sum_t taps[t] v'[m+t] / alpha - alpha * u'[m] / beta_old    (first = 0)
 // or first = 1:  u' = b / 1024 (the right-hand side), nothing else.
-// 4 (u) and 3 (v) CTAs per SM: measured optimum on B200 (1 / 2 / 4 / 6 for u: 872 / 887 / 784 / 1165 ms per configs[2] block of
-// 25 iterations; more spills, fewer leaves too few loads in flight)
-__global__ void __launch_bounds__(kLsmrThreads, 4) u_kernel(float *u, long long upitch, long long n_eq, const float *v,
+// Groups of 8 rows and 4 CTAs per SM for both kernels: measured optimum on B200 (ms per configs[2] block of 25 iterations,
+// group / CTAs of u / CTAs of v: 16/1/1 872, 16/4/3 705, 8/4/4 672, 8/5/4 783, 8/6/5 1009, 4/4/4 716, 12/4/4 695, 32/2/2 845)
+__global__ void __launch_bounds__(kLsmrThreads, LOFAR_U_MINB) u_kernel(float *u, long long upitch, long long n_eq, const float *v,
                                                          long long vpitch, const float *gs, const Scal *sc, double *partial,
                                                          int nchunks, int first)
 {
@@ -55,21 +65,21 @@ __global__ void __launch_bounds__(kLsmrThreads, 4) u_kernel(float *u, long long 
         // rows in groups of 16: the 16 new rows of v' and the 16 rows of u' are loaded before anything is computed (32
         // independent loads per thread in flight -- the kernel is a stream and lives on memory-level parallelism); the
         // window w[0..30] = v'[mb .. mb+30] slides by 16 registers per group
-        float tap[kTapsN], w[2 * kTapsN - 1];
+        float tap[kTapsN], w[kTapsN - 1 + kG];
 #pragma unroll
         for (int t = 0; t < kTapsN; ++t) tap[t] = gs[t * kRes + r] * (1.0f / 1024.0f);
 #pragma unroll
         for (int t = 0; t < kTapsN - 1; ++t) w[t] = pv[(size_t)(m0 + t) * kRes];
-        for (long long mb = m0; mb < m1; mb += kTapsN) {
-            float un[kTapsN];
+        for (long long mb = m0; mb < m1; mb += kG) {
+            float un[kG];
 #pragma unroll
-            for (int k = 0; k < kTapsN; ++k) {
+            for (int k = 0; k < kG; ++k) {
                 const bool ok = mb + k < m1;                     // rows m .. m+15 of v' exist for m < n_eq (n_un = n_eq + 15)
                 w[kTapsN - 1 + k] = ok ? pv[(size_t)(mb + k + kTapsN - 1) * kRes] : 0.f;
                 un[k] = ok ? pu[(size_t)(mb + k) * kRes] : 0.f;
             }
 #pragma unroll
-            for (int k = 0; k < kTapsN; ++k) {
+            for (int k = 0; k < kG; ++k) {
                 float acc = 0.f;
 #pragma unroll
                 for (int t = 0; t < kTapsN; ++t) acc = fmaf(tap[t], w[k + t], acc);
@@ -80,14 +90,14 @@ __global__ void __launch_bounds__(kLsmrThreads, 4) u_kernel(float *u, long long 
                 }
             }
 #pragma unroll
-            for (int t = 0; t < kTapsN - 1; ++t) w[t] = w[t + kTapsN];
+            for (int t = 0; t < kTapsN - 1; ++t) w[t] = w[t + kG];
         }
     }
     partial[((size_t)series * nchunks + chunk) * kRes + r] = s;
 }
 
 // v'[n] = sum_t taps[t] u'[n-t] / beta - beta * v'[n] / alpha_old     (first: no second term)
-__global__ void __launch_bounds__(kLsmrThreads, 3) v_kernel(float *v, long long vpitch, long long n_un, const float *u,
+__global__ void __launch_bounds__(kLsmrThreads, LOFAR_V_MINB) v_kernel(float *v, long long vpitch, long long n_un, const float *u,
                                                          long long upitch, long long n_eq, const float *gs, const Scal *sc,
                                                          double *partial, int nchunks, int first)
 {
@@ -98,7 +108,7 @@ __global__ void __launch_bounds__(kLsmrThreads, 3) v_kernel(float *v, long long 
     const Scal z = sc[(size_t)series * kRes + r];
     const float ib = (float)z.inv_beta, ba = first ? 0.f : (float)(z.beta * z.inv_alpha);
     // as u_kernel: groups of 16 rows, loads first. w[j] = u'[nb - 15 + j], j = 0..30 (zero outside 0 .. n_eq-1)
-    float tap[kTapsN], w[2 * kTapsN - 1];
+    float tap[kTapsN], w[kTapsN - 1 + kG];
 #pragma unroll
     for (int t = 0; t < kTapsN; ++t) tap[t] = gs[t * kRes + r] * (1.0f / 1024.0f);
 #pragma unroll
@@ -107,16 +117,16 @@ __global__ void __launch_bounds__(kLsmrThreads, 3) v_kernel(float *v, long long 
         w[j] = (m >= 0 && m < n_eq) ? pu[(size_t)m * kRes] : 0.f;
     }
     double s = 0.0;
-    for (long long nb = n0; nb < n1; nb += kTapsN) {
-        float vo[kTapsN];
+    for (long long nb = n0; nb < n1; nb += kG) {
+        float vo[kG];
 #pragma unroll
-        for (int k = 0; k < kTapsN; ++k) {
+        for (int k = 0; k < kG; ++k) {
             const long long n = nb + k;
             w[kTapsN - 1 + k] = (n < n1 && n < n_eq) ? pu[(size_t)n * kRes] : 0.f;
             vo[k] = (!first && n < n1) ? pv[(size_t)n * kRes] : 0.f;
         }
 #pragma unroll
-        for (int k = 0; k < kTapsN; ++k) {
+        for (int k = 0; k < kG; ++k) {
             float acc = 0.f;
 #pragma unroll
             for (int t = 0; t < kTapsN; ++t) acc = fmaf(tap[t], w[kTapsN - 1 + k - t], acc);    // u'[n - t]
@@ -128,7 +138,7 @@ __global__ void __launch_bounds__(kLsmrThreads, 3) v_kernel(float *v, long long 
             }
         }
 #pragma unroll
-        for (int j = 0; j < kTapsN - 1; ++j) w[j] = w[j + kTapsN];
+        for (int j = 0; j < kTapsN - 1; ++j) w[j] = w[j + kG];
     }
     partial[((size_t)series * nchunks + chunk) * kRes + r] = s;
 }
