@@ -119,6 +119,42 @@ __global__ void __launch_bounds__(256) scan_kernel(TriggerArgs a)
         const long long c = all ? it % a.nchunks : a.items[it].y;
         const long long n0 = c * kChunk;
         const long long n1 = (n0 + kChunk < a.N) ? n0 + kChunk : a.N;
+        if (a.W == 1 && D == 1) {
+            // one series per beam, envelope = |x|: four rows of 256 samples are loaded before any is judged (when the
+            // flag list overflowed the whole series streams through here)
+            const float *x = a.series + (size_t)b * a.series_pitch;
+            const float sig = a.sigma_thr[b];
+            for (long long nb = n0; nb < n1; nb += 1024) {
+                float ev[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const long long n = nb + u * 256 + threadIdx.x;
+                    ev[u] = n < n1 ? fabsf(x[n]) : -1.f;
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const long long n = nb + u * 256 + threadIdx.x;
+                    const bool hit = ev[u] >= 0.f && ev[u] / sig > a.kappa;
+                    const unsigned mask = __ballot_sync(0xffffffffu, hit);
+                    if (mask) {
+                        unsigned base = 0;
+                        if (lane == 0) base = atomicAdd(a.count, (unsigned)__popc(mask));
+                        base = __shfl_sync(0xffffffffu, base, 0);
+                        if (hit) {
+                            const unsigned slot = base + __popc(mask & ((1u << lane) - 1u));
+                            if (slot < a.cap) {
+                                lofar_candidate r;
+                                r.series = (uint32_t)b; r.trial = 0u;
+                                r.sample = a.offset + (uint64_t)n;
+                                r.env = ev[u]; r.sigma = sig;
+                                a.cand[slot] = r;
+                            }
+                        }
+                    }
+                }
+            }
+            continue;
+        }
         for (long long nb = n0; nb < n1; nb += 256) {
             const long long n = nb + threadIdx.x;
             bool hit = false;
