@@ -212,6 +212,10 @@ def _close(got, ref, what, rel, mx):
     (dict(S=4, B=2, K=16, k0=300, T=72, dtype="ci16", n_pulses=2, blocks=2, kappa=4.0), 25),
     (dict(S=4, B=3, K=488, k0=24, T=200, dtype="ci8", n_pulses=3, blocks=2, kappa=4.5), 25),
     (dict(S=3, B=2, K=24, k0=100, T=40, dtype="ci8", stec=(8.0, 12.0), n_pulses=2, blocks=2, kappa=4.0), 7),
+    # even and minimal iteration counts: the x update is applied every other iteration, the last one must not be lost
+    (dict(S=3, B=2, K=24, k0=100, T=56, dtype="ci8", n_pulses=2, blocks=2, kappa=4.0), 8),
+    (dict(S=3, B=2, K=24, k0=100, T=56, dtype="ci8", n_pulses=2, blocks=2, kappa=4.0), 2),
+    (dict(S=3, B=2, K=24, k0=100, T=56, dtype="ci8", n_pulses=2, blocks=2, kappa=4.0), 1),
 ])
 def test_lsmr_inversion_parity(torch, oracle, kw, iters):
     """LOFAR_INV_LSMR against O11 (= scipy's lsmr, pinned): whole chain, two blocks (the 15 carried slices are rows of
