@@ -190,12 +190,15 @@ __global__ void __launch_bounds__(kLsmrThreads) scalar_kernel(Scal *sc, const do
 // term of the previous iteration, cxp * hbar_old, then this one -- the same two fused multiply-adds in the same order
 // as two separate updates, so the result is bit-identical.
 __global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, float *x, const float *v, long long pitch,
-                                                         long long n_un, const Scal *sc, int first, int xmode)
+                                                         long long n_un, const Scal *sc, int first, int xmode,
+                                                         float *series, long long series_pitch, long long T)
 {
-    const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, series = blockIdx.z;
-    const Scal z = sc[(size_t)series * kRes + r];
+    // series != nullptr (the last iteration): the solution leaves through here -- series[q][r] = x[q + 15][r] -- instead
+    // of going back to the work vector and through a copy kernel
+    const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, series_idx = blockIdx.z;
+    const Scal z = sc[(size_t)series_idx * kRes + r];
     const float ia = (float)z.inv_alpha, ch = (float)z.ch, cx = (float)z.cx, cv = (float)z.cv, cxp = (float)z.cxp;
-    const size_t base = (size_t)series * pitch + r;
+    const size_t base = (size_t)series_idx * pitch + r;
     const long long n0 = (long long)chunk * kRows, n1 = n0 + kRows < n_un ? n0 + kRows : n_un;
     for (long long nb = n0; nb < n1; nb += 4) {
         float vv[4], hh[4], hb[4], xx[4];
@@ -218,22 +221,17 @@ __global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, 
             else {
                 const float b = fmaf(-ch, hb[k], hh[k]);
                 hbar[i] = b;
-                if (xmode == 0) x[i] = fmaf(cx, b, xx[k]);
-                else if (xmode == 2) x[i] = fmaf(cx, b, fmaf(cxp, hb[k], xx[k]));
+                if (xmode != 1) {
+                    const float xn = fmaf(cx, b, xmode == 2 ? fmaf(cxp, hb[k], xx[k]) : xx[k]);
+                    if (series) {
+                        const long long q = nb + k - (kTapsN - 1);
+                        if (q >= 0 && q < T) series[(size_t)series_idx * series_pitch + (size_t)q * kRes + r] = xn;
+                    } else x[i] = xn;
+                }
                 h[i] = fmaf(-cv, hh[k], vn);
             }
         }
     }
-}
-
-// series[q][r] = x[q + 15][r]
-__global__ void __launch_bounds__(kLsmrThreads) out_kernel(const float *x, long long pitch, float *series, long long series_pitch,
-                                                           long long T)
-{
-    const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, s = blockIdx.z;
-    const long long q0 = (long long)chunk * kRows, q1 = q0 + kRows < T ? q0 + kRows : T;
-    for (long long q = q0; q < q1; ++q)
-        series[(size_t)s * series_pitch + (size_t)q * kRes + r] = x[(size_t)s * pitch + (size_t)(q + kTapsN - 1) * kRes + r];
 }
 
 }  // namespace
@@ -258,7 +256,7 @@ int launch_lsmr(float *y, long long ypitch, long long T, float *work, long long 
     scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, ce, 0); ++n;
     v_kernel<<<gu, kLsmrThreads, 0, st>>>(v, wpitch, n_un, y, ypitch, n_eq, gs, sc, partial, cu, 1); ++n;
     scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, cu, 1); ++n;
-    h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 1, 0); ++n;
+    h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 1, 0, nullptr, 0, 0); ++n;
     bool pending = false;                               // an x update of the previous iteration is still to be applied
     for (int k = 0; k < iters; ++k) {
         u_kernel<<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 0); ++n;
@@ -266,11 +264,10 @@ int launch_lsmr(float *y, long long ypitch, long long T, float *work, long long 
         v_kernel<<<gu, kLsmrThreads, 0, st>>>(v, wpitch, n_un, y, ypitch, n_eq, gs, sc, partial, cu, 0); ++n;
         scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, cu, 3); ++n;
         const int xmode = pending ? 2 : (k == iters - 1 ? 0 : 1);
-        h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 0, xmode); ++n;
+        const bool last = (k == iters - 1);              // the last update writes the solution straight into the series
+        h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 0, xmode, last ? series : nullptr, series_pitch, T); ++n;
         pending = (xmode == 1);
     }
-    const dim3 go(kRes / kLsmrThreads, (unsigned)((T + kRows - 1) / kRows), nseries);
-    out_kernel<<<go, kLsmrThreads, 0, st>>>(x, wpitch, series, series_pitch, T); ++n;
     return cudaGetLastError() == cudaSuccess ? n : -1;
 }
 
