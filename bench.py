@@ -369,7 +369,7 @@ def run_gpu(args, idx=None):
         ("beamform", w.S * 2 * w.K * w.T * esz + B * w.K * w.T * 8),
         ("ippf_kernel", B * w.K * w.T * 8 + (ninv * w.T * w.M * 4 if (out_series or mode in ("lsmr", "exact")) else 0)),
         ("trigger", ns * (w.T // 16) * 12 + (2 * ns * w.T * w.M * 4 if mode in ("lsmr", "exact") else 0)),
-        ("lsmr (25 iterations)", ninv * w.T * w.M * 4 * (2 + 12 * 25)),      # u: 3, v: 3, h: 5 or 7 vector passes per iteration
+        ("lsmr (25 iterations)", ninv * w.T * w.M * 4 * (8 + 11 * 25)),      # per iteration: v pass 3, u pass 3 + h/hbar/x 4 or 6
         ("dedisp_kernel", (B * 16 / 14 + ns) * w.T * w.M * 4),
     ]
     tc = w.dtype == "ci8" and B >= 4 and w.S <= 32

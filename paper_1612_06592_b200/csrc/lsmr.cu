@@ -25,6 +25,9 @@ constexpr int kLsmrThreads = 256;
 #ifndef LOFAR_U_MINB
 #define LOFAR_U_MINB 4
 #endif
+#ifndef LOFAR_UH_MINB
+#define LOFAR_UH_MINB 2
+#endif
 #ifndef LOFAR_V_MINB
 #define LOFAR_V_MINB 4
 #endif
@@ -44,9 +47,13 @@ __device__ __forceinline__ double safe_div(double a, double d) { return d != 0.0
 // or first = 1:  u' = b / 1024 (the right-hand side), nothing else.
 // Groups of 8 rows and 4 CTAs per SM for both kernels: measured optimum on B200 (ms per configs[2] block of 25 iterations,
 // group / CTAs of u / CTAs of v: 16/1/1 872, 16/4/3 705, 8/4/4 672, 8/5/4 783, 8/6/5 1009, 4/4/4 716, 12/4/4 695, 32/2/2 845)
-__global__ void __launch_bounds__(kLsmrThreads, LOFAR_U_MINB) u_kernel(float *u, long long upitch, long long n_eq, const float *v,
-                                                         long long vpitch, const float *gs, const Scal *sc, double *partial,
-                                                         int nchunks, int first)
+// HM >= 0: the h / hbar / x update of the PREVIOUS iteration (h_kernel with xmode = HM) is done here for rows 0 .. n_eq-1,
+// on the v' values this kernel holds in its window anyway -- v' is then read once per iteration instead of twice; the
+// last 15 rows (n_eq .. n_un-1) are left to a small h_kernel launch.  h, hbar, x share the pitch of v'.
+template <int HM>
+__global__ void __launch_bounds__(kLsmrThreads, HM >= 0 ? LOFAR_UH_MINB : LOFAR_U_MINB)
+u_kernel(float *u, long long upitch, long long n_eq, const float *v, long long vpitch, const float *gs, const Scal *sc,
+         double *partial, int nchunks, int first, float *h, float *hbar, float *x)
 {
     const int r = blockIdx.x * kLsmrThreads + threadIdx.x, chunk = blockIdx.y, series = blockIdx.z;
     float *pu = u + (size_t)series * upitch + r;
@@ -70,13 +77,35 @@ __global__ void __launch_bounds__(kLsmrThreads, LOFAR_U_MINB) u_kernel(float *u,
         for (int t = 0; t < kTapsN; ++t) tap[t] = gs[t * kRes + r] * (1.0f / 1024.0f);
 #pragma unroll
         for (int t = 0; t < kTapsN - 1; ++t) w[t] = pv[(size_t)(m0 + t) * kRes];
+        const float ch = (float)z.ch, cx = (float)z.cx, cv = (float)z.cv, cxp = (float)z.cxp;
+        const size_t hbase = (size_t)series * vpitch + r;
         for (long long mb = m0; mb < m1; mb += kG) {
-            float un[kG];
+            float un[kG], hh[HM >= 0 ? kG : 1], hb[HM >= 0 ? kG : 1], xx[(HM == 0 || HM == 2) ? kG : 1];
 #pragma unroll
             for (int k = 0; k < kG; ++k) {
                 const bool ok = mb + k < m1;                     // rows m .. m+15 of v' exist for m < n_eq (n_un = n_eq + 15)
                 w[kTapsN - 1 + k] = ok ? pv[(size_t)(mb + k + kTapsN - 1) * kRes] : 0.f;
                 un[k] = ok ? pu[(size_t)(mb + k) * kRes] : 0.f;
+                if (HM >= 0) {
+                    const size_t i = hbase + (size_t)(mb + k) * kRes;
+                    hh[k] = ok ? h[i] : 0.f;
+                    hb[k] = ok ? hbar[i] : 0.f;
+                    if (HM == 0 || HM == 2) xx[k] = ok ? x[i] : 0.f;
+                }
+            }
+            if (HM >= 0) {
+#pragma unroll
+                for (int k = 0; k < kG; ++k) {
+                    if (mb + k < m1) {
+                        const size_t i = hbase + (size_t)(mb + k) * kRes;
+                        const float vn = w[k] * ia;              // v' of row mb + k
+                        const float b = fmaf(-ch, hb[k], hh[k]);
+                        hbar[i] = b;
+                        if (HM == 0) x[i] = fmaf(cx, b, xx[k]);
+                        if (HM == 2) x[i] = fmaf(cx, b, fmaf(cxp, hb[k], xx[k]));
+                        h[i] = fmaf(-cv, hh[k], vn);
+                    }
+                }
             }
 #pragma unroll
             for (int k = 0; k < kG; ++k) {
@@ -191,7 +220,7 @@ __global__ void __launch_bounds__(kLsmrThreads) scalar_kernel(Scal *sc, const do
 // as two separate updates, so the result is bit-identical.
 __global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, float *x, const float *v, long long pitch,
                                                          long long n_un, const Scal *sc, int first, int xmode,
-                                                         float *series, long long series_pitch, long long T)
+                                                         float *series, long long series_pitch, long long T, long long n_begin)
 {
     // series != nullptr (the last iteration): the solution leaves through here -- series[q][r] = x[q + 15][r] -- instead
     // of going back to the work vector and through a copy kernel
@@ -199,7 +228,7 @@ __global__ void __launch_bounds__(kLsmrThreads) h_kernel(float *h, float *hbar, 
     const Scal z = sc[(size_t)series_idx * kRes + r];
     const float ia = (float)z.inv_alpha, ch = (float)z.ch, cx = (float)z.cx, cv = (float)z.cv, cxp = (float)z.cxp;
     const size_t base = (size_t)series_idx * pitch + r;
-    const long long n0 = (long long)chunk * kRows, n1 = n0 + kRows < n_un ? n0 + kRows : n_un;
+    const long long n0 = n_begin + (long long)chunk * kRows, n1 = n0 + kRows < n_un ? n0 + kRows : n_un;
     for (long long nb = n0; nb < n1; nb += 4) {
         float vv[4], hh[4], hb[4], xx[4];
 #pragma unroll
@@ -252,21 +281,31 @@ int launch_lsmr(float *y, long long ypitch, long long T, float *work, long long 
     const dim3 ge(kRes / kLsmrThreads, ce, nseries), gu(kRes / kLsmrThreads, cu, nseries), gs2(kRes / kLsmrThreads, nseries);
     int n = 0;
     cudaMemsetAsync(sc, 0, lsmr_scalar_bytes(nseries), st);
-    u_kernel<<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 1); ++n;
+    u_kernel<-1><<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 1, nullptr, nullptr, nullptr); ++n;
     scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, ce, 0); ++n;
     v_kernel<<<gu, kLsmrThreads, 0, st>>>(v, wpitch, n_un, y, ypitch, n_eq, gs, sc, partial, cu, 1); ++n;
     scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, cu, 1); ++n;
-    h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 1, 0, nullptr, 0, 0); ++n;
-    bool pending = false;                               // an x update of the previous iteration is still to be applied
+    h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 1, 0, nullptr, 0, 0, 0); ++n;
+    // The h / hbar / x update of iteration k-1 rides on the u pass of iteration k (rows 0 .. n_eq-1) plus a 15-row launch;
+    // x is updated every other iteration (xmode 1 = deferred, 2 = two terms); the last update is a full h_kernel that
+    // writes the solution straight into the series.
+    const dim3 gtail(kRes / kLsmrThreads, 1, nseries);
+    int hm = -1;                                        // x-mode of the update that is still to be done, -1: none
+    bool pending = false;                               // an x term of an earlier iteration is still to be applied
     for (int k = 0; k < iters; ++k) {
-        u_kernel<<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 0); ++n;
+        if (hm == 1) u_kernel<1><<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 0, h, hbar, x);
+        else if (hm == 2) u_kernel<2><<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 0, h, hbar, x);
+        else u_kernel<-1><<<ge, kLsmrThreads, 0, st>>>(y, ypitch, n_eq, v, wpitch, gs, sc, partial, ce, 0, nullptr, nullptr, nullptr);
+        ++n;
+        if (hm >= 0) { h_kernel<<<gtail, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 0, hm, nullptr, 0, 0, n_eq); ++n; }
         scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, ce, 2); ++n;
         v_kernel<<<gu, kLsmrThreads, 0, st>>>(v, wpitch, n_un, y, ypitch, n_eq, gs, sc, partial, cu, 0); ++n;
         scalar_kernel<<<gs2, kLsmrThreads, 0, st>>>(sc, partial, cu, 3); ++n;
-        const int xmode = pending ? 2 : (k == iters - 1 ? 0 : 1);
-        const bool last = (k == iters - 1);              // the last update writes the solution straight into the series
-        h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 0, xmode, last ? series : nullptr, series_pitch, T); ++n;
+        const bool last = (k == iters - 1);
+        const int xmode = pending ? 2 : (last ? 0 : 1);
         pending = (xmode == 1);
+        if (last) { h_kernel<<<gu, kLsmrThreads, 0, st>>>(h, hbar, x, v, wpitch, n_un, sc, 0, xmode, series, series_pitch, T, 0); ++n; }
+        else hm = xmode;                                 // done by the next u pass
     }
     return cudaGetLastError() == cudaSuccess ? n : -1;
 }
