@@ -30,6 +30,26 @@ constexpr size_t kDdSmem = (size_t)(kSeg * kDdRow + 256 + 512) * sizeof(float2);
 __device__ __forceinline__ float2 cmulf(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ float2 conjf(float2 a) { return make_float2(a.x, -a.y); }
 
+// Twiddle exp(2 pi i tid k1 / 8192) of the 16 x 512 split, k1 = 0..15, from its four binary powers b[i] =
+// exp(2 pi i tid 2^i / 8192): four table loads per thread (strides 1, 2, 4, 8) and at most three products instead of
+// sixteen loads whose stride grows with k1 -- those loads were half of the kernel's L1 traffic (ncu: l1tex 78 % busy).
+template <int K1>
+__device__ __forceinline__ float2 tw_pow(const float2 (&b)[4])
+{
+    float2 w = make_float2(1.f, 0.f);
+    bool have = false;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+        if (K1 & (1 << i)) { w = have ? cmulf(w, b[i]) : b[i]; have = true; }
+    return w;
+}
+template <int K1, typename F>
+__device__ __forceinline__ void for_k1(F &&f, const float2 (&b)[4])
+{
+    f(K1, tw_pow<K1>(b));
+    if constexpr (K1 < 15) for_k1<K1 + 1>(f, b);
+}
+
 // Position of transform element k = k1 + 16 k2 in the rows.
 __device__ __forceinline__ int pos(int k) { return (k & 15) * kDdRow + pad(k >> 4); }
 
@@ -54,10 +74,12 @@ __global__ void __launch_bounds__(kDdThreads, 2) dedisp_kernel(DedispArgs a)
         x[n1] = PK(v.x, -v.y);                                      // conj z
     }
     idft16p(x);
+    float2 bw[4];
 #pragma unroll
-    for (int k1 = 0; k1 < 16; ++k1) {
-        const float2 w = __ldg(a.tw8192 + ((tid * k1) & (kNc - 1)));
-        sts64(rows + k1 * kDdRow + pad(tid), cmulp(x[k1], w.x, w.y));
+    for (int i = 0; i < 4; ++i) bw[i] = __ldg(a.tw8192 + ((tid << i) & (kNc - 1)));
+    {
+        float2 *col = rows + pad(tid);
+        for_k1<0>([&](int k1, float2 w) { sts64(col + k1 * kDdRow, cmulp(x[k1], w.x, w.y)); }, bw);
     }
     __syncthreads();
     fft512_warp(rows + warp * kDdRow, stw, lane);                  // rows now hold conj(FFT z)
@@ -94,10 +116,10 @@ __global__ void __launch_bounds__(kDdThreads, 2) dedisp_kernel(DedispArgs a)
     fft512_warp(rows + warp * kDdRow, stw, lane);
     __syncthreads();
 #pragma unroll
-    for (int k1 = 0; k1 < 16; ++k1) {
-        const float2 w = __ldg(a.tw8192 + ((tid * k1) & (kNc - 1)));
-        const float2 v = rows[k1 * kDdRow + pad(tid)];
-        x[k1] = cmulp(PK(v.x, v.y), w.x, w.y);
+    for (int i = 0; i < 4; ++i) bw[i] = __ldg(a.tw8192 + ((tid << i) & (kNc - 1)));
+    {
+        const float2 *col = rows + pad(tid);
+        for_k1<0>([&](int k1, float2 w) { const float2 v = col[k1 * kDdRow]; x[k1] = cmulp(PK(v.x, v.y), w.x, w.y); }, bw);
     }
     idft16p(x);
     const float scale = 1.0f / 16384.0f;
