@@ -176,7 +176,7 @@ LOFAR_API lofar_status lofar_plan_set_scratch_limit(lofar_plan *plan, size_t byt
  * for 16 SMs fewer (one wave), which the beamformer uses.  The caller's stream forks into the two lanes and
  * joins them again inside the call, so stream order as seen by the caller is unchanged.  The series are
  * bit-identical to mode 0; sigma differs in its summation order only.  Measured on B200:
- * slower than mode 0 for configs[2] (10.2 vs 9.9 ms per block) because the beamformer needs ~40 SMs' worth of
+ * slower than mode 0 for configs[2] (9.8 - 10.1 vs 9.2 ms per block) because the beamformer needs ~40 SMs' worth of
  * issue slots to reach its HBM rate -- kept as an option, off by default. */
 LOFAR_API lofar_status lofar_plan_set_overlap(lofar_plan *plan, int mode, int chunk_slices);
 /* How lofar_run_block would cut a block of `slices`: slices per scratch chunk, and the number and
