@@ -9,7 +9,9 @@ honours. Switches: LOFAR_FIR_PACKED (synthesis FIR with packed FFMA2 instead of 
 transform's complex adds / butterflies as scalar pairs instead of FADD2 / FFMA2), LOFAR_ST_PLAIN (series stores with
 the default cache policy instead of st.global.cs), LOFAR_ABLATE_STORES
 (inverse PPF without its series stores), LOFAR_ABLATE_FIR (no FIR arithmetic), LOFAR_ABLATE_FFT (no transform
-arithmetic). Ablated variants compute wrong results by design; they exist to attribute time.
+arithmetic). Ablated variants compute wrong results by design; they exist to attribute time. Extra nvcc flags for an
+experiment go in the environment variable LOFAR_NVCC_FLAGS (e.g. "-Xptxas --allow-expensive-optimizations=true": measured, no
+effect).
 """
 from __future__ import annotations
 
@@ -49,7 +51,8 @@ def build(force: bool = False, verbose: bool = False, defines=(), out: str | Non
     for s in SOURCES:
         o = os.path.join(objdir, s.replace(".cu", ".o"))
         objs.append(o)
-        cmd = [NVCC, *FLAGS, *[f"-D{d}" for d in defines], "-c", os.path.join(CSRC, s), "-o", o]
+        cmd = [NVCC, *FLAGS, *os.environ.get("LOFAR_NVCC_FLAGS", "").split(), *[f"-D{d}" for d in defines], "-c",
+               os.path.join(CSRC, s), "-o", o]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         procs.append((s, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
