@@ -46,12 +46,20 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!mbar_try_wait(bar, parity)) {}
 }
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
 {
@@ -216,13 +224,16 @@ __device__ __forceinline__ u64 fir_fma(u64 g, u64 x, u64 acc)
 // 0..15, column pn; FULL = all 16 output slices valid (no predicates on the fast path).
 template <bool FULL>
 __device__ __forceinline__ void fir_step(const float2 *prev, const float2 *cur, const u64 (&g)[kP], int pn, float *out,
-                                         int tid, int nvalid, u64 &ssum2, float &smax)
+                                         int tid, int nvalid, u64 &ssum2, float &smax, uint32_t bar_b = 0, uint32_t phase_b = 0)
 {
     u64 acc[kStep];
 #pragma unroll
     for (int j = 0; j < kStep; ++j) acc[j] = 0ull;
 #pragma unroll
     for (int i = 0; i < kP - 1 + kStep; ++i) {
+        // the 15 carried rows need nothing of this step: the warps only wait for each other's radix-32 pass here, with
+        // almost half of the FIR's arithmetic already issued (split barrier: arrive after pass B, wait before row 0)
+        if (i == kP - 1 && bar_b) mbar_wait(bar_b, phase_b);
         const u64 x = lds64((i < kP - 1) ? prev + (i + 1) * kRow + pn : cur + (i - (kP - 1)) * kRow + pn);
 #pragma unroll
         for (int t = 0; t < kP; ++t) {
@@ -260,6 +271,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     float *sred = reinterpret_cast<float *>(sph + kH + 1);         // 16 floats, 16 doubles, the mbarrier
     double *sdred = reinterpret_cast<double *>(sred + 16);
     const uint32_t bar = smem_u32(sdred + 16);
+    const uint32_t bar_b = bar + 8;                                // "radix-32 pass done": one arrival per warp and step
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int series = blockIdx.x % a.nseries;
@@ -275,6 +287,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 
     if (tid == 0) {
         mbar_init(bar, 1);
+        mbar_init(bar_b, kThreads / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = tid; i < kTwCount; i += kThreads) stw[i] = a.tw[i];
@@ -303,7 +316,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 
     // the first step of a span that starts inside the block is a warm-up: transform the 16 slices before it
     const int q_first = span == 0 ? qs : qs - kStep;
-    uint32_t phase = 0;
+    uint32_t phase = 0, phase_b = 0;
     bool async = stage_fill(a, Zs, q_first, stage_k, bar, tid);
 
     double dsum = 0.0;
@@ -321,9 +334,11 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 #ifndef LOFAR_ABLATE_FFT
         fft512_pass_b<false>(cur + warp * kRow, stw, lane);
 #endif
-        __syncthreads();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_b);       // waited for where the rows of this step are first read
 
         if (q >= qs && a.yout) {
+            mbar_wait(bar_b, phase_b);
             // LSMR inversion (f1): hand the inverse-DFT rows to the solver instead of applying the matched FIR
             float *yout = a.yout + (size_t)series * a.yout_pitch + a.out0;
             const int nvalid = (qe - q < kStep) ? qe - q : kStep;
@@ -344,8 +359,10 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
             float smax = 0.f;
             float *o = a.series ? a.series + (size_t)series * a.series_pitch + a.out0 + (size_t)q * kM : nullptr;
 #ifndef LOFAR_ABLATE_FIR
-            if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
-            else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax);
+            if (nvalid == kStep) fir_step<true>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax, bar_b, phase_b);
+            else fir_step<false>(prev, cur, g, pn, o, tid, nvalid, ssum2, smax, bar_b, phase_b);
+#else
+            mbar_wait(bar_b, phase_b);
 #endif
             if (smax > thr)
                 emit_step(prev, cur, a.gs, tid, pn, nvalid, a.cand, a.count, a.cap, (uint32_t)series, (uint32_t)(series % a.D),
@@ -372,6 +389,11 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
                 a.chunkmax[(size_t)series * a.chunkmax_pitch + a.step0 + q / kStep] = m;
             }
         }
+        else {
+            mbar_wait(bar_b, phase_b);           // warm-up step: nothing reads the rows, the buffers swap below
+            __syncthreads();
+        }
+        phase_b ^= 1;
         float2 *t = prev; prev = cur; cur = t;
     }
 
