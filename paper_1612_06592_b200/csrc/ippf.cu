@@ -136,7 +136,8 @@ __device__ __forceinline__ void vpair(u64 a, u64 b, float2 w, u64 &vm, u64 &vmir
 // place further (fixed up below), bin 0 keeps its real part only and pairs with the always-zero row 512 (reading A10),
 // and bin 256 is its own mirror. One code path for all warps keeps the loop body inside the instruction cache.
 template <bool PH>
-__device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, float2 *dst, const float2 *stw, int tid)
+__device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, float2 *dst, const float2 *stw, int tid,
+                                       uint32_t bar_f = 0, uint32_t phase_f = 0)
 {
     const int warp = tid >> 5, lane = tid & 31, half = lane >> 4, t = lane & 15;
     constexpr int R = 32 * kStep;                  // stage elements between bins m and m + 32
@@ -168,6 +169,9 @@ __device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, f
     const float2 *T = stw + 256 + 16 * j;          // T[m] = TBs[j][m] = +-exp(2 pi i j m / 512), minus for j = 3 (mod 4)
     float2 *row = dst + t * kRow + 17 * j;         // pad(16 j + m) = 17 j + m
     if ((j & 3) == 3) x[0] = PK(-LO(x[0]), -HI(x[0]));      // TBs[j][0] = -1: the one twiddle that is not loaded
+    // dst still holds the carried rows the FIR of the previous step reads: wait for all warps to be through with it
+    // only now, with the loads, the pair pre-pass and the butterflies of this step done (split barrier)
+    if (bar_f) mbar_wait(bar_f, phase_f);
     sts64(row, x[0]);
 #pragma unroll
     for (int m = 1; m < 16; ++m) {
@@ -272,6 +276,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     double *sdred = reinterpret_cast<double *>(sred + 16);
     const uint32_t bar = smem_u32(sdred + 16);
     const uint32_t bar_b = bar + 8;                                // "radix-32 pass done": one arrival per warp and step
+    const uint32_t bar_f = bar + 16;                               // "through with the previous step's rows": the same
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int series = blockIdx.x % a.nseries;
@@ -288,6 +293,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     if (tid == 0) {
         mbar_init(bar, 1);
         mbar_init(bar_b, kThreads / 32);
+        mbar_init(bar_f, kThreads / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = tid; i < kTwCount; i += kThreads) stw[i] = a.tw[i];
@@ -316,7 +322,8 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
 
     // the first step of a span that starts inside the block is a warm-up: transform the 16 slices before it
     const int q_first = span == 0 ? qs : qs - kStep;
-    uint32_t phase = 0, phase_b = 0;
+    uint32_t phase = 0, phase_b = 0, phase_f = 1;     // phase_f = 1: nothing to wait for before the first step
+    int pend = -1;                                   // step whose maximum is still in sred (written out after the next pass A)
     bool async = stage_fill(a, Zs, q_first, stage_k, bar, tid);
 
     double dsum = 0.0;
@@ -326,10 +333,20 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
         if (async) { while (!mbar_try_wait(bar, phase)) {} phase ^= 1; }
         else __syncthreads();
 #ifndef LOFAR_ABLATE_FFT
-        if (trials) pass_a<true>(stage, sph, cur, stw, tid);
-        else pass_a<false>(stage, sph, cur, stw, tid);
+        if (trials) pass_a<true>(stage, sph, cur, stw, tid, bar_f, phase_f);
+        else pass_a<false>(stage, sph, cur, stw, tid, bar_f, phase_f);
+#else
+        mbar_wait(bar_f, phase_f);
 #endif
+        phase_f ^= 1;
         __syncthreads();                         // radix-16 results of all 16 slices in cur, stage free
+        if (pend >= 0 && tid == 0) {             // every warp has passed bar_f: sred of the previous step is complete
+            float m = sred[0];
+#pragma unroll
+            for (int w = 1; w < kThreads / 32; ++w) m = fmaxf(m, sred[w]);
+            a.chunkmax[(size_t)series * a.chunkmax_pitch + a.step0 + pend] = m;
+        }
+        pend = -1;
         if (q + kStep < qe) async = stage_fill(a, Zs, q + kStep, stage_k, bar, tid);   // flies during pass B + FIR
 #ifndef LOFAR_ABLATE_FFT
         fft512_pass_b<false>(cur + warp * kRow, stw, lane);
@@ -352,7 +369,8 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
                     *reinterpret_cast<float2 *>(h + (size_t)idx * kM + 2 * tid) = v;
                 }
             }
-            __syncthreads();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_f);
         } else if (q >= qs) {
             const int nvalid = (qe - q < kStep) ? qe - q : kStep;
             u64 ssum2 = 0ull;
@@ -381,17 +399,14 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
                     *reinterpret_cast<float2 *>(h + (size_t)idx * kM + 2 * tid) = v;
                 }
             }
-            __syncthreads();
-            if (tid == 0) {
-                float m = sred[0];
-#pragma unroll
-                for (int w = 1; w < kThreads / 32; ++w) m = fmaxf(m, sred[w]);
-                a.chunkmax[(size_t)series * a.chunkmax_pitch + a.step0 + q / kStep] = m;
-            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_f);   // waited for in the next pass A, before it overwrites the carried rows
+            pend = q / kStep;
         }
         else {
             mbar_wait(bar_b, phase_b);           // warm-up step: nothing reads the rows, the buffers swap below
-            __syncthreads();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_f);
         }
         phase_b ^= 1;
         float2 *t = prev; prev = cur; cur = t;
@@ -402,6 +417,12 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
     for (int s = 16; s > 0; s >>= 1) dsum += __shfl_xor_sync(0xffffffffu, dsum, s);
     if (lane == 0) sdred[warp] = dsum;
     __syncthreads();
+    if (tid == 0 && pend >= 0) {
+        float m = sred[0];
+#pragma unroll
+        for (int w = 1; w < kThreads / 32; ++w) m = fmaxf(m, sred[w]);
+        a.chunkmax[(size_t)series * a.chunkmax_pitch + a.step0 + pend] = m;
+    }
     if (tid == 0) {
         double s = 0.0;
         for (int w = 0; w < kThreads / 32; ++w) s += sdred[w];
