@@ -169,15 +169,16 @@ __device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, f
     const float2 *T = stw + 256 + 16 * j;          // T[m] = TBs[j][m] = +-exp(2 pi i j m / 512), minus for j = 3 (mod 4)
     float2 *row = dst + t * kRow + 17 * j;         // pad(16 j + m) = 17 j + m
     if ((j & 3) == 3) x[0] = PK(-LO(x[0]), -HI(x[0]));      // TBs[j][0] = -1: the one twiddle that is not loaded
-    // dst still holds the carried rows the FIR of the previous step reads: wait for all warps to be through with it
-    // only now, with the loads, the pair pre-pass and the butterflies of this step done (split barrier)
-    if (bar_f) mbar_wait(bar_f, phase_f);
-    sts64(row, x[0]);
 #pragma unroll
     for (int m = 1; m < 16; ++m) {
         const float2 f = T[m];
-        sts64(row + m, cmulp(x[m], f.x, f.y));
+        x[m] = cmulp(x[m], f.x, f.y);
     }
+    // dst still holds the carried rows the FIR of the previous step reads: wait for all warps to be through with it
+    // only now, with everything of this step but its 16 stores done (split barrier)
+    if (bar_f) mbar_wait(bar_f, phase_f);
+#pragma unroll
+    for (int m = 0; m < 16; ++m) sts64(row + m, x[m]);
 }
 
 // Rare path, kept out of line and out of the FIR's registers: a thread whose step maximum exceeds the threshold
