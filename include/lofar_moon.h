@@ -278,6 +278,26 @@ LOFAR_API lofar_status lofar_plan_profile_read(lofar_plan *plan, double *ms_host
 LOFAR_API uint64_t lofar_plan_launch_count(const lofar_plan *plan);
 LOFAR_API const char *lofar_status_string(lofar_status status);
 
+/* ---- allocation-free entry point -------------------------------------------------------------------
+ * The stand-alone trigger of lofar_trigger (step a5: sigma = RMS of |x| over the block per series, candidates
+ * |x| / sigma > kappa, sorted by (series, sample); one trial per series, env_window 1) for callers that may not
+ * allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  It takes no
+ * plan and calls no cudaMalloc / cudaFree or allocating library routine: its scratch (per-chunk sums and maxima,
+ * the list of flagged chunks) is a fixed file-scope device array of about 6.1 MiB that every GPU holding the
+ * library keeps until the process exits.  Limit: ceil(samples / 16384) * nseries <= LOFAR_STATIC_MAX_CHUNKS
+ * (e.g. 24 series of 131072 slices = 196608 chunks); beyond it the call returns LOFAR_E_SHAPE ("shape out of
+ * range") and launches nothing.
+ * series[nseries][series_pitch] (device, series_pitch >= samples, in floats), cand[max_candidates], count[1],
+ * sigma[nseries]: device buffers of the caller; offset = global index of sample 0.  Work is enqueued on `stream`;
+ * no synchronisation.  Overflow rule as lofar_trigger (R1): *count is the true total.
+ * The array is shared by all calls (all threads, all streams) and keeps the last call's contents; every call clears
+ * what must start at zero on its own stream.  Calls that overlap on the GPU race on it: order them (one stream, or
+ * events between streams). */
+#define LOFAR_STATIC_MAX_CHUNKS 524288
+LOFAR_API lofar_status lofar_trigger_static(const float *series, int nseries, int64_t samples, int64_t series_pitch,
+                                            double kappa, uint64_t offset, lofar_candidate *cand,
+                                            uint32_t max_candidates, uint32_t *count, float *sigma, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

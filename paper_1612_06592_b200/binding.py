@@ -42,7 +42,7 @@ EXPORTS = (
     "lofar_stream_get_state", "lofar_stream_set_state", "lofar_beamform_dedisperse",
     "lofar_inverse_ppf", "lofar_trigger", "lofar_run_block", "lofar_stream_reset",
     "lofar_stream_push", "lofar_stream_sync", "lofar_plan_profile", "lofar_plan_profile_read",
-    "lofar_plan_launch_count", "lofar_status_string",
+    "lofar_plan_launch_count", "lofar_status_string", "lofar_trigger_static",
 )
 
 
@@ -101,6 +101,7 @@ def load() -> ctypes.CDLL:
         "lofar_plan_profile_read": (i, [vp, vp, vp]),
         "lofar_plan_launch_count": (u64, [vp]),
         "lofar_status_string": (c.c_char_p, [i]),
+        "lofar_trigger_static": (i, [vp, i, c.c_int64, c.c_int64, d, u64, vp, u32, vp, vp, vp]),
     }
     for name, (res, args) in sig.items():
         f = getattr(lib, name)
@@ -333,6 +334,18 @@ def plan_for(w, tau) -> Plan:
     p.set_input(LOFAR_CI16 if w.dtype == "ci16" else LOFAR_CI8, w.T)
     p.set_trigger(w.kappa, 1, 65536)
     return p
+
+
+STATIC_MAX_CHUNKS = 524288       # LOFAR_STATIC_MAX_CHUNKS of include/lofar_moon.h
+
+
+def trigger_static(series, samples: int, kappa: float, cand, count, sigma, offset: int = 0, stream=None, allow=()):
+    """lofar_trigger_static: the allocation-free trigger on series[nseries][pitch] (torch tensors of the caller)."""
+    lib = load()
+    nseries, pitch = int(series.shape[0]), int(series.stride(0))
+    return _check(lib.lofar_trigger_static(_ptr(series), nseries, int(samples), pitch, float(kappa), int(offset), _ptr(cand),
+                                           int(cand.shape[0]), _ptr(count), _ptr(sigma), _stream_ptr(stream)),
+                  "lofar_trigger_static", allow)
 
 
 def new_outputs(plan: Plan, slices: int, device="cuda"):

@@ -23,7 +23,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liblofar_moon.so")
-SOURCES = ["api.cu", "beamform.cu", "beamform_tc.cu", "ippf.cu", "trigger.cu", "lsmr.cu", "dedisp.cu"]
+SOURCES = ["api.cu", "beamform.cu", "beamform_tc.cu", "ippf.cu", "trigger.cu", "lsmr.cu", "dedisp.cu", "noalloc.cu"]
 HEADERS = ["plan.h", "fft_math.cuh", "fft_warp.cuh", os.path.join(ROOT, "include", "lofar_moon.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
