@@ -100,6 +100,13 @@ __device__ __forceinline__ bool stage_fill(const IppfArgs &a, const float2 *Zs, 
     return false;
 }
 
+// Twiddles into shared memory: w1024[j + 32 r] goes to stw[8 j + r] (the 8 values a pass-A thread needs side by side),
+// the radix-32 table TBs[32][16] follows unchanged at stw + 256.
+__device__ __forceinline__ void load_twiddles(float2 *stw, const float2 *tw, int tid)
+{
+    for (int i = tid; i < kTwCount; i += kThreads) stw[i < 256 ? 8 * (i & 31) + (i >> 5) : i] = tw[i];
+}
+
 // ---- pass A: pair pre-pass fused with the radix-16 pass of the 512-point transform ---------------------
 // The stage is indexed by the absolute bin: row m holds the 16 slices of bin m; the rows of unselected bins are
 // zeroed once per CTA (reading A10) and the copies only ever write rows k0 .. k0 + K - 1, so the transform reads
@@ -145,7 +152,18 @@ __device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, f
     const bool dc = (warp | half) == 0;            // the thread that holds bins 0, 32, ..., 480
     u64 x[16];
     const float2 *sa = stage + j * kStep + t, *sb = stage + (512 - j) * kStep + t;
-    const float2 *pa = sph + j, *pb = sph + 512 - j, *wj = stw + j;
+    const float2 *pa = sph + j, *pb = sph + 512 - j;
+    // the 8 pair twiddles w^(j + 32 r) of this thread sit side by side (load_twiddles) and come in as four 16-byte loads
+    float2 wj[8];
+    {
+        const float4 *w4 = reinterpret_cast<const float4 *>(stw + 8 * j);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const float4 v = w4[r];
+            wj[2 * r] = make_float2(v.x, v.y);
+            wj[2 * r + 1] = make_float2(v.z, v.w);
+        }
+    }
     u64 give[8];
     {
         u64 a0 = ldz<PH>(sa, pa);
@@ -153,7 +171,7 @@ __device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, f
         vpair(a0, ldz<PH>(sb, pb), wj[0], x[0], give[0]);
     }
 #pragma unroll
-    for (int r = 1; r < 8; ++r) vpair(ldz<PH>(sa + r * R, pa + 32 * r), ldz<PH>(sb - r * R, pb - 32 * r), wj[32 * r], x[r], give[r]);
+    for (int r = 1; r < 8; ++r) vpair(ldz<PH>(sa + r * R, pa + 32 * r), ldz<PH>(sb - r * R, pb - 32 * r), wj[r], x[r], give[r]);
     const int partner = warp ? lane ^ 16 : lane;
 #pragma unroll
     for (int r = 0; r < 8; ++r) x[15 - r] = __shfl_sync(0xffffffffu, give[r], partner);
@@ -169,10 +187,14 @@ __device__ __forceinline__ void pass_a(const float2 *stage, const float2 *sph, f
     const float2 *T = stw + 256 + 16 * j;          // T[m] = TBs[j][m] = +-exp(2 pi i j m / 512), minus for j = 3 (mod 4)
     float2 *row = dst + t * kRow + 17 * j;         // pad(16 j + m) = 17 j + m
     if ((j & 3) == 3) x[0] = PK(-LO(x[0]), -HI(x[0]));      // TBs[j][0] = -1: the one twiddle that is not loaded
+    {
+        const float4 *T4 = reinterpret_cast<const float4 *>(T);      // (T[m], T[m + 1]) per 16-byte load; T is 128-byte aligned
 #pragma unroll
-    for (int m = 1; m < 16; ++m) {
-        const float2 f = T[m];
-        x[m] = cmulp(x[m], f.x, f.y);
+        for (int m = 0; m < 16; m += 2) {
+            const float4 f = T4[m >> 1];
+            if (m) x[m] = cmulp(x[m], f.x, f.y);
+            x[m + 1] = cmulp(x[m + 1], f.z, f.w);
+        }
     }
     // dst still holds the carried rows the FIR of the previous step reads: wait for all warps to be through with it
     // only now, with everything of this step but its 16 stores done (split barrier)
@@ -297,7 +319,7 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
         mbar_init(bar_f, kThreads / 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int i = tid; i < kTwCount; i += kThreads) stw[i] = a.tw[i];
+    load_twiddles(stw, a.tw, tid);
     for (int i = tid; i < kStageF2; i += kThreads) stage[i] = make_float2(0.f, 0.f);   // unselected bins stay zero
     if (trials) {
         const float2 *ph = a.Dph + (size_t)(series % a.zmap_trials) * a.K;
@@ -475,7 +497,7 @@ __global__ void __launch_bounds__(kThreads, 1) rescan_kernel(RescanArgs r)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t total = *r.nitems < r.items_cap ? *r.nitems : r.items_cap;
     if (blockIdx.x >= total) return;
-    for (int i = tid; i < kTwCount; i += kThreads) stw[i] = r.tw[i];
+    load_twiddles(stw, r.tw, tid);
     for (int i = tid; i < kStageF2; i += kThreads) stage[i] = make_float2(0.f, 0.f);
     sph[tid] = make_float2(1.f, 0.f);
     if (tid == 0) sph[kH] = make_float2(1.f, 0.f);
