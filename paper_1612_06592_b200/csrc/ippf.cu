@@ -22,6 +22,9 @@
 // register-file limited). Launch parameters are read from the constant bank where they are used and slice indices
 // are 32-bit, which keeps the persistent register state small: the kernel sits at the 128-register cap and every
 // register the scheduler gets back shows in the FIR.
+// Synchronisation per step: one full barrier (after pass A: every warp writes into every slice row) and two split
+// ones on mbarriers -- warps arrive after pass B and the FIR waits only before it reads the first row of the current
+// step (the 15 carried rows are applied first); warps arrive after the FIR and pass A waits only before its stores.
 // The 15-slice history lives in the "previous" buffer, is loaded from the plan at the start of a block and
 // written back by the CTA that owns the last span; CTAs that start in the middle of a block first
 // transform the 16 slices before their span (no output).
