@@ -365,13 +365,15 @@ __global__ void __launch_bounds__(kThreads, 1) ippf_kernel(IppfArgs a)
         mbar_wait(bar_f, phase_f);
 #endif
         phase_f ^= 1;
-        __syncthreads();                         // radix-16 results of all 16 slices in cur, stage free
-        if (pend >= 0 && tid == 0) {             // every warp has passed bar_f: sred of the previous step is complete
+        // Thread 0 has waited on bar_f inside pass A: every warp has arrived there, i.e. written its maximum of the
+        // previous step into sred; and no warp can write the next one before the barrier below, which needs thread 0.
+        if (pend >= 0 && tid == 0) {
             float m = sred[0];
 #pragma unroll
             for (int w = 1; w < kThreads / 32; ++w) m = fmaxf(m, sred[w]);
             a.chunkmax[(size_t)series * a.chunkmax_pitch + a.step0 + pend] = m;
         }
+        __syncthreads();                         // radix-16 results of all 16 slices in cur, stage free
         pend = -1;
         if (q + kStep < qe) async = stage_fill(a, Zs, q + kStep, stage_k, bar, tid);   // flies during pass B + FIR
 #ifndef LOFAR_ABLATE_FFT
